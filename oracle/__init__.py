@@ -1,0 +1,167 @@
+"""CPU oracle for the SDM coalescence hot path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes access to ``oracle/sdm_oracle.c`` (plain C, fp64, single thread, written from the
+paper).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package; the product (``paper_2101_06318_b200``)
+never does, and this package imports nothing from the product.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+KERNEL_GOLOVIN = 0
+KERNEL_GRAVITATIONAL = 1
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        L = _lib
+        p = C.c_void_p
+        L.orc_philox4x32_10.argtypes = [p, p, p]
+        L.orc_philox4x32_10.restype = None
+        L.orc_rng.argtypes = [C.c_int64, p, C.c_uint64, C.c_uint64, p, p]
+        L.orc_rng.restype = None
+        L.orc_cell_start.argtypes = [C.c_int64, p, C.c_int32, p]
+        L.orc_cell_start.restype = C.c_int
+        L.orc_permutation.argtypes = [C.c_int64, p, p, p, p]
+        L.orc_permutation.restype = None
+        L.orc_cbrt_spec.argtypes = [C.c_double]
+        L.orc_cbrt_spec.restype = C.c_double
+        L.orc_kernel.argtypes = [C.c_int32, C.c_double, C.c_double, C.c_double]
+        L.orc_kernel.restype = C.c_double
+        L.orc_pair_probability.argtypes = [C.c_double, C.c_int64, C.c_int64, C.c_double, C.c_double]
+        L.orc_pair_probability.restype = C.c_double
+        L.orc_gamma_tilde.argtypes = [C.c_double, C.c_double, C.c_int64, C.c_int64]
+        L.orc_gamma_tilde.restype = C.c_int64
+        L.orc_collide_pair.argtypes = [p, p, p, p, C.c_int64]
+        L.orc_collide_pair.restype = None
+        L.orc_step.argtypes = [C.c_int64, p, p, p, C.c_int32, p, C.c_double, C.c_double, C.c_int32,
+                               C.c_double, C.c_uint64, C.c_uint64, p, p, p]
+        L.orc_step.restype = C.c_int
+        L.orc_remove_zero.argtypes = [C.c_int64, p, p, p]
+        L.orc_remove_zero.restype = C.c_int64
+        L.orc_moments.argtypes = [C.c_int64, p, p, p, C.c_int32, C.c_int32, p, p, p]
+        L.orc_moments.restype = None
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _chk(a, dtype):
+    assert isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous, (a.dtype, dtype)
+    return a
+
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox4x32_10(_ptr(c), _ptr(k), _ptr(out))
+    return out
+
+
+def rng(n, seed, step, sid=None):
+    key64 = np.empty(n, dtype=np.uint64)
+    ucand = np.empty(n, dtype=np.float64)
+    if sid is not None:
+        sid = _chk(np.ascontiguousarray(sid, dtype=np.int64), np.int64)
+    lib().orc_rng(n, _ptr(sid), seed, step, _ptr(key64), _ptr(ucand))
+    return key64, ucand
+
+
+def cell_start(cell_id, n_cell) -> np.ndarray:
+    cell_id = _chk(cell_id, np.int32)
+    cs = np.empty(n_cell + 1, dtype=np.int32)
+    rc = lib().orc_cell_start(cell_id.shape[0], _ptr(cell_id), n_cell, _ptr(cs))
+    if rc != 0:
+        raise ValueError("cell id out of range")
+    return cs
+
+
+def permutation(cell_id, key64, sid=None) -> np.ndarray:
+    cell_id = _chk(cell_id, np.int32)
+    key64 = _chk(key64, np.uint64)
+    if sid is not None:
+        sid = _chk(np.ascontiguousarray(sid, dtype=np.int64), np.int64)
+    idx = np.empty(cell_id.shape[0], dtype=np.int32)
+    lib().orc_permutation(cell_id.shape[0], _ptr(cell_id), _ptr(key64), _ptr(sid), _ptr(idx))
+    return idx
+
+
+def cbrt_spec(x: float) -> float:
+    return lib().orc_cbrt_spec(float(x))
+
+
+def kernel(ktype: int, kparam: float, vj: float, vk: float) -> float:
+    return lib().orc_kernel(ktype, float(kparam), float(vj), float(vk))
+
+
+def pair_probability(K: float, xi_max: int, n_s: int, dt: float, dV: float) -> float:
+    return lib().orc_pair_probability(float(K), int(xi_max), int(n_s), float(dt), float(dV))
+
+
+def gamma_tilde(p: float, u: float, xi_j: int, xi_k: int) -> int:
+    return lib().orc_gamma_tilde(float(p), float(u), int(xi_j), int(xi_k))
+
+
+def collide_pair(xi_a: int, v_a: float, xi_b: int, v_b: float, gamma: int):
+    """Fig. 5 body for the pair (first, second) with uncapped gamma -> (xi_a, v_a, xi_b, v_b)."""
+    xa, xb = C.c_int64(xi_a), C.c_int64(xi_b)
+    va, vb = C.c_double(v_a), C.c_double(v_b)
+    lib().orc_collide_pair(C.byref(xa), C.byref(va), C.byref(xb), C.byref(vb), int(gamma))
+    return xa.value, va.value, xb.value, vb.value
+
+
+def step(xi, v, cell_id, n_cell, dt, dV, ktype, kparam, seed, step, sid=None, want_perm=True):
+    """One coalescence step IN PLACE on (xi, v).  Returns (idx, cell_start, n_events)."""
+    xi = _chk(xi, np.int64)
+    v = _chk(v, np.float64)
+    cell_id = _chk(cell_id, np.int32)
+    n = xi.shape[0]
+    assert v.shape[0] == n and cell_id.shape[0] == n
+    if sid is not None:
+        sid = _chk(np.ascontiguousarray(sid, dtype=np.int64), np.int64)
+    idx = np.empty(n, dtype=np.int32) if want_perm else None
+    cs = np.empty(n_cell + 1, dtype=np.int32) if want_perm else None
+    nev = C.c_int64(0)
+    rc = lib().orc_step(n, _ptr(xi), _ptr(v), _ptr(cell_id), n_cell, _ptr(sid), float(dt), float(dV),
+                        int(ktype), float(kparam), int(seed), int(step), _ptr(idx), _ptr(cs),
+                        C.byref(nev))
+    if rc != 0:
+        raise ValueError("orc_step: invalid input")
+    return idx, cs, nev.value
+
+
+def remove_zero(xi, v, cell_id):
+    """Stable removal of xi == 0.  Returns trimmed COPIES (xi, v, cell_id)."""
+    xi = _chk(xi, np.int64).copy()
+    v = _chk(v, np.float64).copy()
+    cell_id = _chk(cell_id, np.int32).copy()
+    m = lib().orc_remove_zero(xi.shape[0], _ptr(xi), _ptr(v), _ptr(cell_id))
+    return xi[:m].copy(), v[:m].copy(), cell_id[:m].copy()
+
+
+def moments(xi, v, cell_id=None, n_cell=1, per_cell=False):
+    xi = _chk(xi, np.int64)
+    v = _chk(v, np.float64)
+    nout = n_cell if per_cell else 1
+    if per_cell:
+        cell_id = _chk(cell_id, np.int32)
+    m0 = np.zeros(nout, dtype=np.int64)
+    m1 = np.zeros(nout, dtype=np.float64)
+    m2 = np.zeros(nout, dtype=np.float64)
+    lib().orc_moments(xi.shape[0], _ptr(xi), _ptr(v), _ptr(cell_id) if per_cell else None,
+                      n_cell, 1 if per_cell else 0, _ptr(m0), _ptr(m1), _ptr(m2))
+    if per_cell:
+        return m0, m1, m2
+    return int(m0[0]), float(m1[0]), float(m2[0])

@@ -1,0 +1,306 @@
+/* sdm_oracle.c -- plain CPU oracle for one SDM coalescence timestep.  See sdm_oracle.h.
+ *
+ * TEST INFRASTRUCTURE ONLY: never linked into, imported by or called from the product path.
+ * Written from the paper (PAPER.md = arXiv 2101.06318) step by step, in the paper's order and
+ * notation; no blocking, fusion or reordering.  Build: gcc -O2 -ffp-contract=off -fPIC -shared.
+ */
+#include "sdm_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------------------------------
+ * Philox4x32-10 (R6; the paper only says "random numbers").
+ * One round:  (hi0,lo0) = M0*c0, (hi1,lo1) = M1*c2,
+ *             c' = { hi1^c1^k0, lo1, hi0^c3^k1, lo0 };  the key is bumped by the Weyl
+ * constants between rounds (before rounds 2..10).
+ * ------------------------------------------------------------------------------------------ */
+#define PHILOX_M0 0xD2511F53u
+#define PHILOX_M1 0xCD9E8D57u
+#define PHILOX_W0 0x9E3779B9u
+#define PHILOX_W1 0xBB67AE85u
+
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += PHILOX_W0; k1 += PHILOX_W1; }
+        uint64_t p0 = (uint64_t)PHILOX_M0 * c0;
+        uint64_t p1 = (uint64_t)PHILOX_M1 * c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* DESIGN.md R6: counter = {sid lo, sid hi, step lo, step hi}, key = {seed lo, seed hi};
+ * sort key = words 0-1, pair uniform = 53 top bits of words 2-3, times 2^-53 (phi ~ U[0,1),
+ * PAPER.md:102). */
+void orc_rng(int64_t n, const int64_t *sid, uint64_t seed, uint64_t step,
+             uint64_t *key64, double *ucand)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        uint64_t s = (uint64_t)(sid ? sid[i] : i);
+        uint32_t ctr[4] = { (uint32_t)s, (uint32_t)(s >> 32), (uint32_t)step, (uint32_t)(step >> 32) };
+        uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+        uint32_t w[4];
+        orc_philox4x32_10(ctr, key, w);
+        key64[i] = (uint64_t)w[0] | ((uint64_t)w[1] << 32);
+        uint64_t bits = (uint64_t)w[2] | ((uint64_t)w[3] << 32);
+        ucand[i] = (double)(bits >> 11) * 0x1.0p-53;
+    }
+}
+
+/* PAPER.md:151 "cell_start = Storage(N_CELL + 1, int)". */
+int orc_cell_start(int64_t n, const int32_t *cell_id, int32_t n_cell, int32_t *cell_start)
+{
+    for (int32_t c = 0; c <= n_cell; ++c) cell_start[c] = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        if (cell_id[i] < 0 || cell_id[i] >= n_cell) return -1;
+        cell_start[cell_id[i] + 1] += 1;                 /* count of cell c at slot c+1 */
+    }
+    for (int32_t c = 0; c < n_cell; ++c) cell_start[c + 1] += cell_start[c];
+    return 0;
+}
+
+/* Step 1: the GPU backend of the paper permutes by sorting on a
+ * random key with the cell id as the major key.  Ties on the key are broken by storage index
+ * (R7). */
+typedef struct { int32_t cell; uint64_t key; int64_t sid; int32_t pos; } orc_rec_t;
+
+static int orc_rec_cmp(const void *pa, const void *pb)
+{
+    const orc_rec_t *a = (const orc_rec_t *)pa, *b = (const orc_rec_t *)pb;
+    if (a->cell != b->cell) return a->cell < b->cell ? -1 : 1;
+    if (a->key != b->key) return a->key < b->key ? -1 : 1;
+    if (a->sid != b->sid) return a->sid < b->sid ? -1 : 1;
+    return 0;
+}
+
+void orc_permutation(int64_t n, const int32_t *cell_id, const uint64_t *key64,
+                     const int64_t *sid, int32_t *idx)
+{
+    orc_rec_t *rec = (orc_rec_t *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_rec_t));
+    for (int64_t i = 0; i < n; ++i) {
+        rec[i].cell = cell_id[i];
+        rec[i].key = key64[i];
+        rec[i].sid = sid ? sid[i] : i;
+        rec[i].pos = (int32_t)i;
+    }
+    qsort(rec, (size_t)n, sizeof(orc_rec_t), orc_rec_cmp);
+    for (int64_t i = 0; i < n; ++i) idx[i] = rec[i].pos;
+    free(rec);
+}
+
+/* DESIGN.md R10: cube root as a fixed sequence of IEEE double operations (libm's cbrt is not
+ * correctly rounded, so it cannot be part of a bit-exact contract).
+ *   y0 = bits -> double( MAGIC - bits(x)/3 )            ~ x^(-1/3), |rel err| < 3.5e-2
+ *   4 x Newton for x^(-1/3):  y <- y * (4/3 - (1/3) * (x*(y*y*y)))
+ *   r  = (x*y)*y                                           ~ x^(1/3)
+ *   r <- r - ((r*r)*r - x) * ((y*y) * (1/3))               one Newton step for r^3 = x
+ * Every product and sum is rounded separately (no FMA).  Result within 1 ulp of the true
+ * cube root for positive normal x (checked in tests/test_oracle_kernels.py). */
+double orc_cbrt_spec(double x)
+{
+    uint64_t bits;
+    memcpy(&bits, &x, sizeof bits);
+    uint64_t ybits = 0x553EEEEEEEEEF000ull - bits / 3ull;
+    double y;
+    memcpy(&y, &ybits, sizeof y);
+    const double c43 = 0x1.5555555555555p+0;   /* 4/3 rounded */
+    const double c13 = 0x1.5555555555555p-2;   /* 1/3 rounded */
+    for (int it = 0; it < 4; ++it) {
+        double t = y * y;
+        t = t * y;
+        t = x * t;
+        t = c13 * t;
+        t = c43 - t;
+        y = y * t;
+    }
+    double r = x * y;
+    r = r * y;
+    double d = r * r;
+    d = d * r;
+    d = d - x;
+    double h = y * y;
+    h = h * c13;
+    d = d * h;
+    r = r - d;
+    return r;
+}
+
+/* Terminal velocity of BASELINE.json config 3 (Rogers-Yau three-regime fit); R9:
+ * the middle branch owns r = 40 um, the top branch owns r = 600 um. */
+static double orc_terminal_velocity(double r)
+{
+    if (r < 40e-6) { double t = 1.19e8 * r; return t * r; }
+    if (r < 600e-6) return 8e3 * r;
+    return 220.0 * sqrt(r);
+}
+
+double orc_kernel(int32_t type, double kparam, double vj, double vk)
+{
+    if (type == ORC_KERNEL_GOLOVIN) {
+        /* a(v1, v2) = b (v1 + v2) */
+        double s = vj + vk;
+        return kparam * s;
+    }
+    /* K = E * pi * (r_j + r_k)^2 * |w_j - w_k|, evaluated left to right; r = cbrt(3 v / (4 pi)) */
+    const double c = 0x1.e8ec8a4aeacc4p-3;     /* 3/(4 pi) */
+    const double pi = 0x1.921fb54442d18p+1;
+    double rj = orc_cbrt_spec(vj * c);
+    double rk = orc_cbrt_spec(vk * c);
+    double wj = orc_terminal_velocity(rj);
+    double wk = orc_terminal_velocity(rk);
+    double s = rj + rk;
+    double s2 = s * s;
+    double K = kparam * pi;
+    K = K * s2;
+    K = K * fabs(wj - wk);
+    return K;
+}
+
+/* Eq. 3:  p = a(v_j,v_k) * max(xi_j,xi_k) * [(n^2-n)/2]/floor(n/2) * dt/dV,
+ * in the order of the routines kernel -> times_max -> normalize. */
+double orc_pair_probability(double K, int64_t xi_max, int64_t n_s, double dt, double dV)
+{
+    double p = K * (double)xi_max;                               /* times_max */
+    int64_t all_pairs = (n_s * (n_s - 1)) / 2;                   /* (n^2 - n)/2 */
+    int64_t cand_pairs = n_s / 2;                                /* floor(n/2) */
+    double norm = (dt / dV) * ((double)all_pairs / (double)cand_pairs);
+    return p * norm;                                             /* normalize */
+}
+
+/* gamma = ceil(p - phi), phi ~ U[0,1) == floor(p) + [phi < p - floor(p)]
+ * (R4); gamma_tilde = min(gamma, floor(xi_j/xi_k)) (Eq. 4).
+ * The comparison with q is made in double first so that a huge p never overflows the
+ * conversion to int64 (R8). */
+int64_t orc_gamma_tilde(double p, double u, int64_t xi_j, int64_t xi_k)
+{
+    double fl = floor(p);
+    double gamma = fl + ((u < p - fl) ? 1.0 : 0.0);
+    int64_t q = xi_j / xi_k;
+    if (fl >= (double)q) return q;
+    int64_t g = (int64_t)gamma;
+    return g < q ? g : q;
+}
+
+/* Fig. 5 for one pair, one attribute. */
+void orc_collide_pair(int64_t *xi_a, double *v_a, int64_t *xi_b, double *v_b, int64_t gamma)
+{
+    int64_t *nj = xi_a, *nk = xi_b;
+    double *aj = v_a, *ak = v_b;
+    if (*nj < *nk) {
+        nj = xi_b; nk = xi_a; aj = v_b; ak = v_a;
+    }
+    if (*nk == 0) return;                             /* DESIGN.md R11: zero-xi partner */
+    int64_t q = *nj / *nk;
+    int64_t g = gamma < q ? gamma : q;                /* PAPER.md:260 (Eq. 4) */
+    if (g == 0) return;
+    int64_t new_n = *nj - g * *nk;
+    if (new_n > 0) {                                  /* Eq. 5 */
+        *nj = new_n;
+        double t = (double)g * *aj;
+        *ak = *ak + t;
+    } else {                                          /* Eq. 6 */
+        *nj = *nk / 2;
+        *nk = *nk - *nj;
+        double t = *aj * (double)g;
+        *aj = t + *ak;
+        *ak = *aj;
+    }
+}
+
+int orc_step(int64_t n, int64_t *xi, double *v, const int32_t *cell_id, int32_t n_cell,
+             const int64_t *sid, double dt, double dV, int32_t kernel, double kparam,
+             uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
+             int64_t *n_events_out)
+{
+    if (n < 0 || n_cell < 1) return -1;
+    uint64_t *key64 = (uint64_t *)malloc((size_t)(n + 1) * sizeof(uint64_t));
+    double *ucand = (double *)malloc((size_t)(n + 1) * sizeof(double));
+    int32_t *idx = (int32_t *)malloc((size_t)(n + 1) * sizeof(int32_t));
+    int32_t *cell_start = (int32_t *)malloc((size_t)(n_cell + 1) * sizeof(int32_t));
+    int64_t n_events = 0;
+    int rc = 0;
+
+    /* step 1: random numbers, cell-wise shuffling */
+    orc_rng(n, sid, seed, step, key64, ucand);
+    if (orc_cell_start(n, cell_id, n_cell, cell_start) != 0) { rc = -1; goto done; }
+    orc_permutation(n, cell_id, key64, sid, idx);
+
+    /* steps 2-3 for every candidate pair (2m, 2m+1) of every cell */
+    for (int32_t c = 0; c < n_cell; ++c) {
+        int64_t s = cell_start[c];
+        int64_t n_s = cell_start[c + 1] - s;
+        for (int64_t m = 0; m < n_s / 2; ++m) {
+            int32_t a = idx[s + 2 * m];               /* first-in-pair */
+            int32_t b = idx[s + 2 * m + 1];
+            int32_t j = a, k = b;
+            if (xi[j] < xi[k]) { j = b; k = a; }
+            if (xi[k] == 0) continue;                 /* DESIGN.md R11 */
+            double K = orc_kernel(kernel, kparam, v[j], v[k]);
+            double p = orc_pair_probability(K, xi[j], n_s, dt, dV);
+            double u = ucand[a];                      /* DESIGN.md R6: uniform of the first member */
+            int64_t g = orc_gamma_tilde(p, u, xi[j], xi[k]);
+            if (g == 0) continue;
+            n_events += 1;
+            /* gamma_tilde <= floor(xi_j/xi_k), so passing it as gamma leaves it unchanged */
+            orc_collide_pair(&xi[a], &v[a], &xi[b], &v[b], g);
+        }
+    }
+    if (idx_out) memcpy(idx_out, idx, (size_t)n * sizeof(int32_t));
+    if (cell_start_out) memcpy(cell_start_out, cell_start, (size_t)(n_cell + 1) * sizeof(int32_t));
+    if (n_events_out) *n_events_out = n_events;
+done:
+    free(key64); free(ucand); free(idx); free(cell_start);
+    return rc;
+}
+
+/* Step 0: filter, order preserved (R12). */
+int64_t orc_remove_zero(int64_t n, int64_t *xi, double *v, int32_t *cell_id)
+{
+    int64_t m = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        if (xi[i] != 0) {
+            xi[m] = xi[i]; v[m] = v[i]; cell_id[m] = cell_id[i];
+            m += 1;
+        }
+    }
+    return m;
+}
+
+/* Neumaier compensated accumulation: sum += x with a running error term. */
+static void orc_acc(double *sum, double *comp, double x)
+{
+    double t = *sum + x;
+    if (fabs(*sum) >= fabs(x)) *comp += (*sum - t) + x;
+    else                       *comp += (x - t) + *sum;
+    *sum = t;
+}
+
+void orc_moments(int64_t n, const int64_t *xi, const double *v, const int32_t *cell_id,
+                 int32_t n_cell, int32_t per_cell, int64_t *m0, double *m1, double *m2)
+{
+    int32_t nout = per_cell ? n_cell : 1;
+    double *c1 = (double *)calloc((size_t)nout, sizeof(double));
+    double *c2 = (double *)calloc((size_t)nout, sizeof(double));
+    for (int32_t c = 0; c < nout; ++c) { m0[c] = 0; m1[c] = 0.0; m2[c] = 0.0; }
+    for (int64_t i = 0; i < n; ++i) {
+        int32_t c = per_cell ? cell_id[i] : 0;
+        double xv = (double)xi[i] * v[i];             /* xi v   */
+        double xvv = xv * v[i];                       /* xi v^2 */
+        m0[c] += xi[i];
+        orc_acc(&m1[c], &c1[c], xv);
+        orc_acc(&m2[c], &c2[c], xvv);
+    }
+    for (int32_t c = 0; c < nout; ++c) { m1[c] += c1[c]; m2[c] += c2[c]; }
+    free(c1); free(c2);
+}
