@@ -1,0 +1,147 @@
+/* sdm.h -- C ABI of libsdm: one Super-Droplet Method (SDM) coalescence timestep on one B200.
+ *
+ * Method: Bartman & Arabas, "On the design of Monte-Carlo particle coagulation solver interface:
+ * a CPU/GPU Super-Droplet Method case study with PySDM", arXiv 2101.06318, cited below as
+ * PAPER.md:<line>.  State of Fig. 2: per super-droplet a multiplicity xi
+ * (int64), one extensive attribute, the volume v (fp64, m^3), and a cell id (int32).  Call order
+ * and in/out intents follow Fig. 3.  Readings of the paper where it is silent
+ * (RNG stream, tie rules, evaluation order, ...) are R1..R14 of DESIGN.md.
+ *
+ * Conventions
+ *  - Every entry point returns an int status: SDM_OK (0) or a negative SDM_E* code.  Nothing
+ *    throws or aborts across this boundary.  sdm_last_error() gives a message for the last failure.
+ *  - "_dev" pointers are DEVICE pointers (CUDA global memory of the current device); "_host"
+ *    pointers are HOST pointers (pinned memory recommended).  The library NEVER allocates device
+ *    memory: the caller supplies one workspace (sdm_workspace_bytes) that must outlive the handle
+ *    ("explicit allocation is used only once per simulation").
+ *  - All device work is enqueued on the cudaStream_t given to sdm_create.  Calls are asynchronous
+ *    with respect to the host unless they return a host value (documented per call).
+ *  - User arrays are caller-owned and only read/written during the call (stream order).
+ *  - Storage order is observable (it feeds the RNG counter and the exported permutation): it is
+ *    the order given to sdm_set_state, then changed only by the stable compaction sdm_remove_zero.
+ *  - There is no CPU fallback: without a CUDA device every compute call fails with SDM_ECUDA.
+ */
+#ifndef SDM_H
+#define SDM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sdm sdm_t; /* opaque handle, owned by the library (host memory only) */
+
+enum { SDM_OK = 0, SDM_EINVAL = -1, SDM_ECAPACITY = -2, SDM_ECUDA = -3, SDM_ESTATE = -4 };
+
+/* Coalescence kernel a(v1, v2) of Eq. 1 / Eq. 3. */
+enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GRAVITATIONAL = 1 };
+typedef struct {
+    int32_t type;     /* SDM_KERNEL_*                                                              */
+    int32_t reserved; /* must be 0                                                                 */
+    double b;         /* Golovin: a = b*(v1+v2), b in 1/s                           */
+    double E;         /* gravitational: a = E*pi*(r1+r2)^2*|w(r1)-w(r2)|, collection efficiency E  */
+                      /* (constants of BASELINE.json config 3, R9-R10)      */
+} sdm_kernel_t;
+
+/* Options for sdm_set_option (testing / profiling; defaults in brackets). */
+enum {
+    SDM_OPT_FORCE_GENERAL = 1, /* [0] 1: never take the cell-contiguous fused path                 */
+    SDM_OPT_SEGMENT_CAP = 2,   /* [0] >0: override the largest segment a warp sorts on chip (tests) */
+    SDM_OPT_WRITE_IDX = 3,     /* [1] 0: do not export the permutation (idx is then undefined)      */
+    SDM_OPT_SCREENING = 4      /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
+};
+
+/* Counter slots returned by sdm_get_counters. */
+enum {
+    SDM_CNT_N_SD = 0,        /* current number of super-droplets                                   */
+    SDM_CNT_EVENTS = 1,      /* pairs with gamma_tilde > 0 since sdm_set_state                      */
+    SDM_CNT_ZEROS = 2,       /* droplets with xi == 0 currently in the state                        */
+    SDM_CNT_LAUNCHES = 3,    /* kernels launched by this handle since sdm_create                    */
+    SDM_CNT_MODE = 4,        /* 0 = general path, 1 = fused cell-contiguous path                    */
+    SDM_CNT_MAX_CELL = 5,    /* largest per-cell count seen at sdm_set_state                        */
+    SDM_CNT_EXACT_EVALS = 6, /* pairs whose Eq. 3 was evaluated in fp64 since sdm_set_state         */
+    SDM_CNT_COUNT = 8
+};
+
+/* Bytes of device workspace needed for `capacity` super-droplets in `n_cell` cells; 0 if the
+ * arguments are invalid (capacity < 1, capacity >= 2^31 - 1024, n_cell < 1). */
+size_t sdm_workspace_bytes(int64_t capacity, int32_t n_cell);
+
+/* Creates a handle.  workspace_dev: caller-owned device memory, 256-byte aligned, at least
+ * sdm_workspace_bytes(capacity, n_cell) bytes.  cuda_stream: a cudaStream_t (NULL = legacy default
+ * stream).  The state is empty (n_sd = 0) until sdm_set_state.  Synchronous (clears the control
+ * block).  Errors: SDM_EINVAL (bad arguments, workspace too small or misaligned), SDM_ECUDA. */
+int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_dev,
+               size_t workspace_bytes, void *cuda_stream);
+
+/* Frees the handle (host memory only; the workspace stays with the caller).  Synchronises the stream. */
+int sdm_destroy(sdm_t *h);
+
+int sdm_set_option(sdm_t *h, int32_t option, int64_t value);
+
+/* Copies a state of n_sd super-droplets into the workspace (Fig. 2: multiplicities, attributes[0],
+ * cell_id), validates it (0 <= cell_id < n_cell, xi >= 0, v finite and > 0) and
+ * analyses its layout (cell-contiguous or not, largest cell).  SYNCHRONOUS.  Errors: SDM_ECAPACITY
+ * (n_sd > capacity), SDM_EINVAL (validation failed; the state is then unusable: SDM_ESTATE later). */
+int sdm_set_state(sdm_t *h, int64_t n_sd, const int64_t *xi_dev, const double *v_dev,
+                  const int32_t *cell_id_dev);
+int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const double *v_host,
+                       const int32_t *cell_id_host);
+
+/* Copies the current state out in storage order.  Any of the array pointers may be NULL.
+ * SYNCHRONOUS (returns n_sd on the host).  The arrays must hold at least n_sd elements (capacity
+ * is always enough). */
+int sdm_get_state(sdm_t *h, int64_t *n_sd, int64_t *xi_dev, double *v_dev, int32_t *cell_id_dev);
+int sdm_get_state_host(sdm_t *h, int64_t *n_sd, int64_t *xi_host, double *v_host,
+                       int32_t *cell_id_host);
+
+/* One coalescence step: Fig. 3 steps 1-3.
+ *   step 1  per-droplet Philox4x32-10 block (counter = storage index and `step`, key = `seed`),
+ *           cell_start table, idx = argsort by (cell_id, key64, storage index)
+ *   step 2  for every candidate pair (idx[s+2m], idx[s+2m+1]) of every cell: Eq. 3
+ *   step 3  gamma = floor(p) + [u < p - floor(p)], gamma_tilde = min(gamma, floor(xi_j/xi_k)) (Eq. 4),
+ *           update of xi and v by Eqs. 5-6 / Fig. 5
+ * dt >= 0 [s], dV > 0 [m^3] (one volume for all cells).  n_sd does not change.
+ * ASYNCHRONOUS.  Errors: SDM_EINVAL (bad dt, dV, kernel), SDM_ESTATE (no valid state), SDM_ECUDA. */
+int sdm_coalescence_step(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
+                         uint64_t step);
+
+/* Step 0 of Fig. 3: removes super-droplets with xi == 0 by a STABLE
+ * compaction of (xi, v, cell_id).  n_sd_out == NULL: ASYNCHRONOUS (n_sd stays on the device);
+ * otherwise SYNCHRONOUS and *n_sd_out receives the new count. */
+int sdm_remove_zero(sdm_t *h, int64_t *n_sd_out);
+
+/* Moments of the size spectrum, M_k = sum xi * v^k for k = 0, 1, 2 (R13).
+ * per_cell == 0: one value each; per_cell != 0: n_cell values each.  M0 is exact (int64); M1, M2
+ * are fp64 sums (products rounded as (xi*v) and (xi*v)*v).  ASYNCHRONOUS for _dev outputs;
+ * the _host variant is SYNCHRONOUS. */
+int sdm_moments(sdm_t *h, int per_cell, int64_t *m0_dev, double *m1_dev, double *m2_dev);
+int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, double *m2_host);
+
+/* Exports the permutation and cell table of the LAST sdm_coalescence_step (parity / debugging;
+ * the paper's `idx` and `cell_start`): idx_dev[n_sd] (storage indices in
+ * cell-major, key-ascending order), cell_start_dev[n_cell + 1].  Either may be NULL.  The copies
+ * are enqueued on the stream; with idx_dev != NULL the call first synchronises to learn n_sd. */
+int sdm_get_permutation(sdm_t *h, int32_t *idx_dev, int32_t *cell_start_dev);
+
+/* n_steps timesteps [sdm_remove_zero (if remove_zero_each_step); sdm_coalescence_step] with
+ * step = step0, step0+1, ...; results equal the per-step calls.  ASYNCHRONOUS. */
+int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
+            uint64_t step0, int64_t n_steps, int remove_zero_each_step);
+
+/* Reads SDM_CNT_COUNT counters into counters_host.  SYNCHRONOUS. */
+int sdm_get_counters(sdm_t *h, int64_t *counters_host);
+
+/* Message for the last error on this handle (never NULL; "" if none).  h may be NULL: then the
+ * message of the last failed sdm_create on this thread. */
+const char *sdm_last_error(const sdm_t *h);
+
+/* ABI version of this header: major*1000 + minor. */
+int sdm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDM_H */

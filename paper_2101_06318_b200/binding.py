@@ -1,0 +1,242 @@
+"""ctypes binding of include/sdm.h -- argument marshalling only.
+
+Every step of the hot path runs inside libsdm.so's CUDA kernels.  Names mirror the C ABI:
+``SDM.set_state`` -> ``sdm_set_state``, ``SDM.coalescence_step`` -> ``sdm_coalescence_step``, ...
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+KERNEL_GOLOVIN = 0
+KERNEL_GRAVITATIONAL = 1
+OPT_FORCE_GENERAL = 1
+OPT_SEGMENT_CAP = 2
+OPT_WRITE_IDX = 3
+OPT_SCREENING = 4
+CNT_NAMES = ("n_sd", "events", "zeros", "launches", "mode", "max_cell", "exact_evals", "reserved")
+
+SDM_OK, SDM_EINVAL, SDM_ECAPACITY, SDM_ECUDA, SDM_ESTATE = 0, -1, -2, -3, -4
+_CODES = {-1: "SDM_EINVAL", -2: "SDM_ECAPACITY", -3: "SDM_ECUDA", -4: "SDM_ESTATE"}
+
+# every symbol include/sdm.h declares (tests check the header against this and the .so)
+SYMBOLS = (
+    "sdm_version", "sdm_workspace_bytes", "sdm_create", "sdm_destroy", "sdm_set_option",
+    "sdm_set_state", "sdm_set_state_host", "sdm_get_state", "sdm_get_state_host",
+    "sdm_coalescence_step", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
+    "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_last_error",
+)
+
+
+class SdmError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_CODES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class KernelDesc(C.Structure):
+    _fields_ = [("type", C.c_int32), ("reserved", C.c_int32), ("b", C.c_double), ("E", C.c_double)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(HERE, "libsdm.so")
+
+
+def load_library() -> C.CDLL:
+    """Loads the in-tree libsdm.so.  Raises (never falls back) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2101_06318_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp, i64, i32, u64, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_uint64, C.c_double
+    L.sdm_version.restype = C.c_int
+    L.sdm_workspace_bytes.argtypes = [i64, i32]
+    L.sdm_workspace_bytes.restype = C.c_size_t
+    L.sdm_create.argtypes = [C.POINTER(vp), i64, i32, vp, C.c_size_t, vp]
+    L.sdm_destroy.argtypes = [vp]
+    L.sdm_set_option.argtypes = [vp, i32, i64]
+    L.sdm_set_state.argtypes = [vp, i64, vp, vp, vp]
+    L.sdm_set_state_host.argtypes = [vp, i64, vp, vp, vp]
+    L.sdm_get_state.argtypes = [vp, C.POINTER(i64), vp, vp, vp]
+    L.sdm_get_state_host.argtypes = [vp, C.POINTER(i64), vp, vp, vp]
+    L.sdm_coalescence_step.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64]
+    L.sdm_remove_zero.argtypes = [vp, C.POINTER(i64)]
+    L.sdm_moments.argtypes = [vp, C.c_int, vp, vp, vp]
+    L.sdm_moments_host.argtypes = [vp, C.c_int, vp, vp, vp]
+    L.sdm_get_permutation.argtypes = [vp, vp, vp]
+    L.sdm_run.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64, i64, C.c_int]
+    L.sdm_get_counters.argtypes = [vp, C.POINTER(i64)]
+    L.sdm_last_error.argtypes = [vp]
+    L.sdm_last_error.restype = C.c_char_p
+    for name in SYMBOLS:
+        if name not in ("sdm_workspace_bytes", "sdm_last_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def version() -> int:
+    return load_library().sdm_version()
+
+
+def workspace_bytes(capacity: int, n_cell: int) -> int:
+    return int(load_library().sdm_workspace_bytes(capacity, n_cell))
+
+
+def _kernel(kernel: int, kparam: float) -> KernelDesc:
+    if kernel == KERNEL_GOLOVIN:
+        return KernelDesc(KERNEL_GOLOVIN, 0, float(kparam), 0.0)
+    return KernelDesc(int(kernel), 0, 0.0, float(kparam))
+
+
+class SDM:
+    """One simulation state on one GPU.  Device memory (workspace) is a torch tensor; the stream is
+    torch's current stream at construction."""
+
+    def __init__(self, capacity: int, n_cell: int, device="cuda:0", stream=None):
+        import torch
+
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: libsdm has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.capacity, self.n_cell = int(capacity), int(n_cell)
+        nbytes = workspace_bytes(self.capacity, self.n_cell)
+        if nbytes == 0:
+            raise SdmError(SDM_EINVAL, "invalid capacity / n_cell")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) // 256 * 256
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            rc = self._lib.sdm_create(C.byref(h), self.capacity, self.n_cell, C.c_void_p(self._ws_ptr),
+                                      nbytes, C.c_void_p(self.stream.cuda_stream))
+        if rc != SDM_OK:
+            raise SdmError(rc, self._lib.sdm_last_error(None).decode())
+        self._h = h
+
+    # -- helpers ------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != SDM_OK:
+            raise SdmError(rc, self._lib.sdm_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._lib.sdm_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @staticmethod
+    def _p(t):
+        return None if t is None else C.c_void_p(t.data_ptr())
+
+    def _dev(self, t, dtype):
+        assert t.is_cuda and t.dtype == dtype and t.is_contiguous(), (t.device, t.dtype)
+        return t
+
+    def _host(self, t, dtype):
+        assert (not t.is_cuda) and t.dtype == dtype and t.is_contiguous(), (t.device, t.dtype)
+        return t
+
+    # -- the C ABI, one method per entry point ---------------------------------------------------
+    def set_option(self, option: int, value: int):
+        self._check(self._lib.sdm_set_option(self._h, option, int(value)))
+
+    def set_state(self, xi, v, cell_id):
+        """xi int64, v float64, cell_id int32 torch tensors on the device."""
+        t = self.torch
+        n = xi.shape[0]
+        self._dev(xi, t.int64), self._dev(v, t.float64), self._dev(cell_id, t.int32)
+        self._check(self._lib.sdm_set_state(self._h, n, self._p(xi), self._p(v), self._p(cell_id)))
+
+    def set_state_host(self, xi, v, cell_id):
+        """Same, from host tensors (pinned recommended): the H2D copies are part of the call."""
+        t = self.torch
+        n = xi.shape[0]
+        self._host(xi, t.int64), self._host(v, t.float64), self._host(cell_id, t.int32)
+        self._check(self._lib.sdm_set_state_host(self._h, n, self._p(xi), self._p(v), self._p(cell_id)))
+
+    def get_state(self):
+        """Returns (xi, v, cell_id) device tensors trimmed to the current n_sd."""
+        t = self.torch
+        xi = t.empty(self.capacity, dtype=t.int64, device=self.device)
+        v = t.empty(self.capacity, dtype=t.float64, device=self.device)
+        c = t.empty(self.capacity, dtype=t.int32, device=self.device)
+        n = C.c_int64(0)
+        self._check(self._lib.sdm_get_state(self._h, C.byref(n), self._p(xi), self._p(v), self._p(c)))
+        return xi[: n.value], v[: n.value], c[: n.value]
+
+    def get_state_host(self, xi, v, cell_id) -> int:
+        """Copies the state into the given host tensors (capacity-sized); returns n_sd."""
+        n = C.c_int64(0)
+        self._check(self._lib.sdm_get_state_host(self._h, C.byref(n), self._p(xi), self._p(v), self._p(cell_id)))
+        return n.value
+
+    def coalescence_step(self, dt, dV, kernel, kparam, seed, step):
+        k = _kernel(kernel, kparam)
+        self._check(self._lib.sdm_coalescence_step(self._h, float(dt), float(dV), C.byref(k), int(seed), int(step)))
+
+    def remove_zero(self, sync: bool = True):
+        if not sync:
+            self._check(self._lib.sdm_remove_zero(self._h, None))
+            return None
+        n = C.c_int64(0)
+        self._check(self._lib.sdm_remove_zero(self._h, C.byref(n)))
+        return n.value
+
+    def moments(self, per_cell: bool = False, out=None):
+        """Device-side moments (asynchronous): returns (m0 int64, m1, m2 float64) device tensors."""
+        t = self.torch
+        k = self.n_cell if per_cell else 1
+        if out is None:
+            out = (t.empty(k, dtype=t.int64, device=self.device), t.empty(k, dtype=t.float64, device=self.device),
+                   t.empty(k, dtype=t.float64, device=self.device))
+        self._check(self._lib.sdm_moments(self._h, 1 if per_cell else 0, self._p(out[0]), self._p(out[1]), self._p(out[2])))
+        return out
+
+    def moments_host(self, per_cell: bool = False):
+        import numpy as np
+
+        k = self.n_cell if per_cell else 1
+        m0 = np.zeros(k, dtype=np.int64)
+        m1 = np.zeros(k, dtype=np.float64)
+        m2 = np.zeros(k, dtype=np.float64)
+        self._check(self._lib.sdm_moments_host(self._h, 1 if per_cell else 0, m0.ctypes.data_as(C.c_void_p),
+                                               m1.ctypes.data_as(C.c_void_p), m2.ctypes.data_as(C.c_void_p)))
+        if per_cell:
+            return m0, m1, m2
+        return int(m0[0]), float(m1[0]), float(m2[0])
+
+    def get_permutation(self, n_sd: int):
+        """(idx[n_sd], cell_start[n_cell+1]) device tensors of the last coalescence step."""
+        t = self.torch
+        idx = t.empty(max(int(n_sd), 1), dtype=t.int32, device=self.device)
+        cs = t.empty(self.n_cell + 1, dtype=t.int32, device=self.device)
+        self._check(self._lib.sdm_get_permutation(self._h, self._p(idx), self._p(cs)))
+        return idx[: int(n_sd)], cs
+
+    def run(self, dt, dV, kernel, kparam, seed, step0, n_steps, remove_zero_each_step=True):
+        k = _kernel(kernel, kparam)
+        self._check(self._lib.sdm_run(self._h, float(dt), float(dV), C.byref(k), int(seed), int(step0),
+                                      int(n_steps), 1 if remove_zero_each_step else 0))
+
+    def counters(self) -> dict:
+        arr = (C.c_int64 * 8)()
+        self._check(self._lib.sdm_get_counters(self._h, arr))
+        return dict(zip(CNT_NAMES, [int(x) for x in arr]))

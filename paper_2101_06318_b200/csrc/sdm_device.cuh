@@ -1,0 +1,172 @@
+// sdm_device.cuh -- device-side arithmetic of the SDM coalescence step (sm_100a).
+//
+// Every floating-point operation whose result reaches the state is written with an explicit
+// round-to-nearest intrinsic (__dmul_rn, __dadd_rn, ...): those are never contracted into FMAs,
+// so the results are bit-identical to a plain IEEE-754 evaluation in the same order (the library
+// is also compiled with -fmad=false).  Citations: PAPER.md = arXiv 2101.06318; R* = DESIGN.md.
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace sdmk {
+
+// ---------------------------------------------------------------------------------------------
+// Row a1: Philox4x32-10, one block per droplet per step (R6).
+// ---------------------------------------------------------------------------------------------
+struct PhiloxKey {          // the ten round keys, precomputed once per thread (uniform values)
+    uint32_t k0[10], k1[10];
+};
+
+__device__ __forceinline__ void philox_round_keys(uint64_t seed, PhiloxKey &rk)
+{
+    uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        rk.k0[r] = a;
+        rk.k1[r] = b;
+        a += 0x9E3779B9u;
+        b += 0xBB67AE85u;
+    }
+}
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKey &rk)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ rk.k0[r];
+        uint32_t n2 = hi0 ^ c3 ^ rk.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// counter = {storage index lo, hi, step lo, hi}; storage index < 2^31 so the hi word is 0
+__device__ __forceinline__ uint4 droplet_block(uint32_t sid, uint64_t step, const PhiloxKey &rk)
+{
+    return philox4x32_10(sid, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
+}
+
+__device__ __forceinline__ uint64_t block_key64(const uint4 &w)
+{
+    return (uint64_t)w.x | ((uint64_t)w.y << 32);
+}
+
+// phi ~ U[0,1): top 53 bits of words 2-3, times 2^-53 (R6)
+__device__ __forceinline__ double block_uniform(const uint4 &w)
+{
+    uint64_t bits = (uint64_t)w.z | ((uint64_t)w.w << 32);
+    return __dmul_rn(__ull2double_rn(bits >> 11), 0x1.0p-53);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a5: coalescence kernels (R9, R10) and Eq. 3.
+// ---------------------------------------------------------------------------------------------
+struct StepParams {
+    double dtdv;      // dt / dV, one IEEE division on the host
+    double kparam;    // Golovin b, or gravitational E
+    int32_t kernel;   // SDM_KERNEL_*
+    int32_t write_idx;
+    uint64_t seed, step;
+    // fp32 screening (see pair_screen): upper bounds, 0 => screening disabled
+    float scr_c;      // upper bound of kparam(*pi)*dt/dV with margin
+    int32_t screening;
+};
+
+// R10: cube root as a fixed sequence of IEEE double operations (no division, no FMA).
+__device__ __forceinline__ double cbrt_spec(double x)
+{
+    uint64_t bits = (uint64_t)__double_as_longlong(x);
+    double y = __longlong_as_double((long long)(0x553EEEEEEEEEF000ull - bits / 3ull));
+    const double c43 = 0x1.5555555555555p+0, c13 = 0x1.5555555555555p-2;
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        double t = __dmul_rn(y, y);
+        t = __dmul_rn(t, y);
+        t = __dmul_rn(x, t);
+        t = __dmul_rn(c13, t);
+        t = __dsub_rn(c43, t);
+        y = __dmul_rn(y, t);
+    }
+    double r = __dmul_rn(__dmul_rn(x, y), y);
+    double d = __dsub_rn(__dmul_rn(__dmul_rn(r, r), r), x);
+    double h = __dmul_rn(__dmul_rn(y, y), c13);
+    return __dsub_rn(r, __dmul_rn(d, h));
+}
+
+__device__ __forceinline__ double terminal_velocity(double r)
+{
+    if (r < 40e-6) return __dmul_rn(__dmul_rn(1.19e8, r), r);
+    if (r < 600e-6) return __dmul_rn(8e3, r);
+    return __dmul_rn(220.0, __dsqrt_rn(r));
+}
+
+__device__ __forceinline__ double coalescence_kernel(int32_t type, double kparam, double vj, double vk)
+{
+    if (type == 0) return __dmul_rn(kparam, __dadd_rn(vj, vk));       // Golovin
+    const double c = 0x1.e8ec8a4aeacc4p-3;                              // 3/(4 pi)
+    const double pi = 0x1.921fb54442d18p+1;
+    double rj = cbrt_spec(__dmul_rn(vj, c));
+    double rk = cbrt_spec(__dmul_rn(vk, c));
+    double wj = terminal_velocity(rj), wk = terminal_velocity(rk);
+    double s = __dadd_rn(rj, rk);
+    double K = __dmul_rn(kparam, pi);
+    K = __dmul_rn(K, __dmul_rn(s, s));
+    return __dmul_rn(K, fabs(__dsub_rn(wj, wk)));
+}
+
+// [(n^2-n)/2] / floor(n/2) is the exact integer n-1 (n even) or n (n odd) (R2), so the quotient
+// of the paper's Eq. 3 needs no division.
+__device__ __forceinline__ double pair_norm(int n_s, double dtdv)
+{
+    int ratio = (n_s & 1) ? n_s : n_s - 1;
+    return __dmul_rn(dtdv, (double)ratio);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Rows a5-a6 for one candidate pair (a = first-in-pair, b = second), in place in global memory.
+// Returns bit 0: an event happened (gamma_tilde > 0); bit 1: a multiplicity became zero.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, double *__restrict__ v,
+                                                  int a, int b, double u, double norm,
+                                                  int32_t ktype, double kparam)
+{
+    int64_t xa = xi[a], xb = xi[b];
+    int j = a, k = b;
+    int64_t xj = xa, xk = xb;
+    if (xa < xb) { j = b; k = a; xj = xb; xk = xa; }     // PAPER.md:257-259 (strict <, R8)
+    if (xk == 0) return 0;                               // R11
+    double vj = v[j], vk = v[k];
+    double K = coalescence_kernel(ktype, kparam, vj, vk);
+    double p = __dmul_rn(__dmul_rn(K, __ll2double_rn(xj)), norm);      // Eq. 3 in routine order (R3)
+    double fl = floor(p);
+    int64_t q = xj / xk;
+    int64_t g;
+    if (fl >= __ll2double_rn(q)) {
+        g = q;                                           // cap reached without converting p (R8)
+    } else {
+        double gamma = (u < __dsub_rn(p, fl)) ? __dadd_rn(fl, 1.0) : fl;   // PAPER.md:102, R4
+        int64_t gi = __double2ll_rz(gamma);
+        g = gi < q ? gi : q;                             // Eq. 4
+    }
+    if (g == 0) return 0;
+    int64_t new_n = xj - g * xk;
+    double gv = __dmul_rn(__ll2double_rn(g), vj);
+    double vnew = __dadd_rn(vk, gv);                     // both branches produce v_k + g v_j
+    if (new_n > 0) {                                     // Eq. 5
+        xi[j] = new_n;
+        v[k] = vnew;
+        return 1;
+    }
+    int64_t half = xk >> 1;                              // Eq. 6, xk > 0
+    xi[j] = half;
+    xi[k] = xk - half;
+    v[j] = vnew;
+    v[k] = vnew;
+    return half == 0 ? 3 : 1;
+}
+
+}  // namespace sdmk

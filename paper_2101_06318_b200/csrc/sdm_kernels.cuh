@@ -1,0 +1,638 @@
+// sdm_kernels.cuh -- CUDA kernels of the SDM coalescence step for sm_100a (rows a1-a8 of the
+// hot-path table in DESIGN.md).  Included once by sdm_api.cu.
+#pragma once
+
+#include "sdm_device.cuh"
+
+namespace sdmk {
+
+constexpr int kWarpCap = 512;            // largest segment one warp sorts in shared memory
+constexpr int kSortWarps = 8;            // warps per CTA in the segment kernels
+constexpr int kCompactTile = 2048;       // elements per compaction tile
+constexpr int kCompactThreads = 256;
+constexpr int kMomentBlocks = 1184;      // 148 SMs x 8
+constexpr int kMomentThreads = 256;
+
+// Device-resident control block: everything the host would otherwise have to synchronise for.
+struct Ctrl {
+    int n;                         // current number of super-droplets
+    int zero_count;                // droplets with xi == 0 in the state
+    int ticket;                    // compaction tile ticket
+    int n_new;                     // compaction result
+    int n_buckets;                 // number of sort segments (split mode)
+    int unsorted;                  // analysis: cell_id decreases somewhere
+    int invalid;                   // analysis: validation failed
+    int max_count;                 // analysis: largest cell
+    unsigned int moment_done;      // moments: last-block counter
+    int pad0;
+    unsigned long long n_events;   // pairs with gamma_tilde > 0
+    unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
+};
+
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+// ---------------------------------------------------------------------------------------------
+// sdm_set_state: validation + layout analysis (not on the per-step path)
+// ---------------------------------------------------------------------------------------------
+__global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restrict__ v,
+                          const int32_t *__restrict__ cell, int n, int n_cell,
+                          int *__restrict__ cell_cnt, Ctrl *ctrl)
+{
+    int zeros = 0, bad = 0, unsorted = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        int c = cell[i];
+        int64_t x = xi[i];
+        double vol = v[i];
+        bool ok = (c >= 0) && (c < n_cell) && (x >= 0) && (vol > 0.0) && (vol < CUDART_INF);
+        if (!ok) { bad = 1; continue; }
+        zeros += (x == 0);
+        if (i > 0 && cell[i - 1] > c) unsorted = 1;
+        atomicAdd(&cell_cnt[c], 1);
+    }
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    bad = __any_sync(0xffffffffu, bad);
+    unsorted = __any_sync(0xffffffffu, unsorted);
+    if (lane_id() == 0) {
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+        if (bad) atomicOr(&ctrl->invalid, 1);
+        if (unsorted) atomicOr(&ctrl->unsorted, 1);
+    }
+}
+
+__global__ void k_max_count(const int *__restrict__ cell_cnt, int n_cell, Ctrl *ctrl)
+{
+    int m = 0;
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cell; c += gridDim.x * blockDim.x)
+        m = max(m, cell_cnt[c]);
+    m = __reduce_max_sync(0xffffffffu, m);
+    if (lane_id() == 0 && m > 0) atomicMax(&ctrl->max_count, m);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a2 (general path): counting sort by cell -- histogram, scan, scatter
+// ---------------------------------------------------------------------------------------------
+__global__ void k_cell_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
+                             int *__restrict__ cell_cnt)
+{
+    const int n = ctrl->n;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+        atomicAdd(&cell_cnt[cell[i]], 1);
+}
+
+// Single-CTA exclusive scan of per-cell counts -> cell_start[n_cell+1].  With split != 0 it also
+// decides, per cell, how many key bits sub-divide the cell into sort segments ("buckets": cells
+// larger than seg_cap are cut by the top bits of the uniform sort key into pieces of mean size
+// in (seg_cap/4, seg_cap/2]) and scans the bucket counts -> bucket_base[n_cell+1].
+constexpr int kScanThreads = 1024;
+constexpr int kScanItems = 8;
+
+__device__ __forceinline__ int block_exclusive_scan(int val, int *s_warp, int &total)
+{
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    int inc = val;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    __syncthreads();
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        int w = s_warp[lane];
+        int winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += t;
+        }
+        s_warp[lane] = winc - w;      // exclusive warp offsets
+        if (lane == 31) s_warp[32] = winc;
+    }
+    __syncthreads();
+    total = s_warp[32];
+    return s_warp[warp] + inc - val;
+}
+
+__device__ __forceinline__ int split_bits(int count, int seg_cap)
+{
+    if (count <= seg_cap) return 0;
+    // smallest B with count / 2^B <= seg_cap/2
+    int target = max(seg_cap >> 1, 1);
+    int B = 0;
+    while (((long long)target << B) < count) ++B;
+    return B;
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_cell_scan(const int *__restrict__ cnt, int n_cell, int *__restrict__ cell_start, int split,
+            int seg_cap, int *__restrict__ cell_bits, int *__restrict__ bucket_base, Ctrl *ctrl)
+{
+    __shared__ int s_warp[33];
+    int carry = 0, bcarry = 0;
+    for (int base = 0; base < n_cell; base += kScanThreads * kScanItems) {
+        int c0 = base + threadIdx.x * kScanItems;
+        int loc[kScanItems], nb[kScanItems];
+        int sum = 0, bsum = 0;
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) {
+            int c = c0 + k;
+            loc[k] = (c < n_cell) ? cnt[c] : 0;
+            int B = split ? split_bits(loc[k], seg_cap) : 0;
+            nb[k] = (c < n_cell) ? (1 << B) : 0;
+            if (split && c < n_cell) cell_bits[c] = B;
+            sum += loc[k];
+            bsum += nb[k];
+        }
+        int total, btotal = 0;
+        int excl = block_exclusive_scan(sum, s_warp, total);
+        int bexcl = 0;
+        if (split) bexcl = block_exclusive_scan(bsum, s_warp, btotal);
+        int run = carry + excl, brun = bcarry + bexcl;
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) {
+            int c = c0 + k;
+            if (c < n_cell) {
+                cell_start[c] = run;
+                if (split) bucket_base[c] = brun;
+            }
+            run += loc[k];
+            brun += nb[k];
+        }
+        carry += total;
+        bcarry += btotal;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        cell_start[n_cell] = carry;
+        if (split) { bucket_base[n_cell] = bcarry; ctrl->n_buckets = bcarry; }
+    }
+}
+
+// bucket of droplet i: its cell's first bucket + the top B bits of its sort key
+__device__ __forceinline__ int bucket_of(int i, int c, const int *__restrict__ cell_bits,
+                                         const int *__restrict__ bucket_base, uint64_t step,
+                                         const PhiloxKey &rk)
+{
+    int B = cell_bits[c];
+    int b = bucket_base[c];
+    if (B > 0) {
+        uint4 w = droplet_block((uint32_t)i, step, rk);
+        b += (int)(w.y >> (32 - B));
+    }
+    return b;
+}
+
+__global__ void k_bucket_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
+                               const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
+                               int *__restrict__ bucket_cnt, uint64_t seed, uint64_t step)
+{
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    const int n = ctrl->n;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+        atomicAdd(&bucket_cnt[bucket_of(i, cell[i], cell_bits, bucket_base, step, rk)], 1);
+}
+
+// exclusive scan of n_buckets counts (n_buckets lives on the device) -> bucket_start[n_buckets+1]
+__global__ void __launch_bounds__(kScanThreads)
+k_bucket_scan(const int *__restrict__ cnt, const Ctrl *__restrict__ ctrl, int *__restrict__ start)
+{
+    __shared__ int s_warp[33];
+    const int nb = ctrl->n_buckets;
+    int carry = 0;
+    for (int base = 0; base < nb; base += kScanThreads * kScanItems) {
+        int c0 = base + threadIdx.x * kScanItems;
+        int loc[kScanItems];
+        int sum = 0;
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) {
+            loc[k] = (c0 + k < nb) ? cnt[c0 + k] : 0;
+            sum += loc[k];
+        }
+        int total;
+        int run = carry + block_exclusive_scan(sum, s_warp, total);
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) {
+            if (c0 + k < nb) start[c0 + k] = run;
+            run += loc[k];
+        }
+        carry += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) start[nb] = carry;
+}
+
+// order[] = droplets grouped by segment (cell, or bucket in split mode); the order inside a
+// segment is arbitrary here -- the segment sort on (key64, storage index) makes it unique.
+__global__ void k_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int split,
+                          const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
+                          const int *__restrict__ seg_start, int *__restrict__ cursor,
+                          int *__restrict__ order, uint64_t seed, uint64_t step)
+{
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    const int n = ctrl->n;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        int c = cell[i];
+        int b = split ? bucket_of(i, c, cell_bits, bucket_base, step, rk) : c;
+        int pos = atomicAdd(&cursor[b], 1);
+        order[seg_start[b] + pos] = i;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a3: per-segment sort by (key64, storage index), one warp per segment, in shared memory
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool key_less(uint64_t ka, int ia, uint64_t kb, int ib)
+{
+    return (ka < kb) || (ka == kb && ia < ib);          // R7: ties by storage index
+}
+
+// bitonic sort of (skey[e], sid[e]), e in [0, N), N a power of two, by one warp
+__device__ __forceinline__ void warp_bitonic(uint64_t *skey, int *sid, int N, int lane)
+{
+    for (int k = 2; k <= N; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = lane; t < (N >> 1); t += 32) {
+                int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                int l = i | j;
+                bool up = (i & k) == 0;
+                uint64_t ka = skey[i], kb = skey[l];
+                int ia = sid[i], ib = sid[l];
+                bool swap = up ? key_less(kb, ib, ka, ia) : key_less(ka, ia, kb, ib);
+                if (swap) { skey[i] = kb; skey[l] = ka; sid[i] = ib; sid[l] = ia; }
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// Never taken with Philox keys and the default cap (a segment would have to exceed its mean by
+// more than 16 standard deviations); kept so that the result is defined for every input:
+// rank by counting, O(m^2) Philox evaluations.
+__device__ __noinline__ void warp_rank_by_counting(const int *__restrict__ ids_in, int contiguous_base,
+                                                   int m, int out_base, int *__restrict__ idx,
+                                                   uint64_t step, const PhiloxKey &rk, int lane)
+{
+    for (int e = lane; e < m; e += 32) {
+        int id = ids_in ? ids_in[e] : contiguous_base + e;
+        uint64_t key = block_key64(droplet_block((uint32_t)id, step, rk));
+        int rank = 0;
+        for (int f = 0; f < m; ++f) {
+            int id2 = ids_in ? ids_in[f] : contiguous_base + f;
+            uint64_t key2 = block_key64(droplet_block((uint32_t)id2, step, rk));
+            rank += key_less(key2, id2, key, id) ? 1 : 0;
+        }
+        idx[out_base + rank] = id;
+    }
+}
+
+// general path: segments described by seg_start[0..n_seg], droplet ids through order[]
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_segment_sort(const int *__restrict__ seg_start, const Ctrl *__restrict__ ctrl, int n_seg_host,
+               int seg_cap, const int *__restrict__ order, int *__restrict__ idx, uint64_t seed,
+               uint64_t step)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    uint64_t *skey = reinterpret_cast<uint64_t *>(smem_raw) + warp * kWarpCap;
+    int *sid = reinterpret_cast<int *>(smem_raw + kSortWarps * kWarpCap * sizeof(uint64_t)) + warp * kWarpCap;
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    const int n_seg = n_seg_host >= 0 ? n_seg_host : ctrl->n_buckets;
+    const int warps_total = gridDim.x * kSortWarps;
+    for (int seg = blockIdx.x * kSortWarps + warp; seg < n_seg; seg += warps_total) {
+        const int s = seg_start[seg];
+        const int m = seg_start[seg + 1] - s;
+        if (m == 0) continue;
+        if (m > seg_cap) {
+            warp_rank_by_counting(order + s, 0, m, s, idx, step, rk, lane);
+            continue;
+        }
+        int N = 2;
+        while (N < m) N <<= 1;
+        for (int e = lane; e < N; e += 32) {
+            if (e < m) {
+                int id = order[s + e];
+                skey[e] = block_key64(droplet_block((uint32_t)id, step, rk));
+                sid[e] = id;
+            } else {
+                skey[e] = ~0ull;
+                sid[e] = 0x7fffffff;
+            }
+        }
+        __syncwarp();
+        warp_bitonic(skey, sid, N, lane);
+        for (int e = lane; e < m; e += 32) idx[s + e] = sid[e];
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Rows a4-a6 (general path): pairs by position in idx, as Fig. 4 flags them
+// ---------------------------------------------------------------------------------------------
+__global__ void k_pairs_by_position(int64_t *__restrict__ xi, double *__restrict__ v,
+                                    const int32_t *__restrict__ cell, const int *__restrict__ idx,
+                                    const int *__restrict__ cell_start, Ctrl *ctrl, StepParams prm)
+{
+    PhiloxKey rk;
+    philox_round_keys(prm.seed, rk);
+    const int n = ctrl->n;
+    int events = 0, zeros = 0;
+    for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
+        int a = idx[p];
+        int c = cell[a];
+        int s = cell_start[c];
+        int n_s = cell_start[c + 1] - s;
+        bool first = (((p - s) & 1) == 0) && (p + 1 < s + n_s);     // Fig. 4
+        if (!first) continue;
+        int b = idx[p + 1];
+        double u = block_uniform(droplet_block((uint32_t)a, prm.step, rk));
+        int r = collide_pair_exact(xi, v, a, b, u, pair_norm(n_s, prm.dtdv), prm.kernel, prm.kparam);
+        events += r & 1;
+        zeros += (r >> 1) & 1;
+    }
+    events = __reduce_add_sync(0xffffffffu, events);
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    if (lane_id() == 0) {
+        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused path (cell-contiguous storage): row a2 by boundary detection, rows a1,a3-a6 per cell
+// ---------------------------------------------------------------------------------------------
+__global__ void k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
+                                    int n_cell, int *__restrict__ cell_start)
+{
+    const int n = ctrl->n;
+    if (n == 0) {
+        for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= n_cell; c += gridDim.x * blockDim.x)
+            cell_start[c] = 0;
+        return;
+    }
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        int c = cell[i];
+        int prev = (i > 0) ? cell[i - 1] : -1;
+        for (int cc = prev + 1; cc <= c; ++cc) cell_start[cc] = i;
+        if (i == n - 1)
+            for (int cc = c + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
+    }
+}
+
+// v1: one warp per cell, (key64, id) bitonic sort in shared memory, pairs read xi/v from global
+__global__ void __launch_bounds__(kSortWarps * 32)
+k_fused_cells_v1(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
+                 int n_cell, int seg_cap, int *__restrict__ idx, Ctrl *ctrl, StepParams prm)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    uint64_t *skey = reinterpret_cast<uint64_t *>(smem_raw) + warp * kWarpCap;
+    int *sid = reinterpret_cast<int *>(smem_raw + kSortWarps * kWarpCap * sizeof(uint64_t)) + warp * kWarpCap;
+    PhiloxKey rk;
+    philox_round_keys(prm.seed, rk);
+    int events = 0, zeros = 0;
+    const int warps_total = gridDim.x * kSortWarps;
+    for (int c = blockIdx.x * kSortWarps + warp; c < n_cell; c += warps_total) {
+        const int s = cell_start[c];
+        const int m = cell_start[c + 1] - s;
+        if (m == 0) continue;
+        const int *sorted = sid;
+        if (m > seg_cap) {   // the host only takes this path when max_count <= seg_cap; kept for safety
+            warp_rank_by_counting(nullptr, s, m, s, idx, prm.step, rk, lane);
+            __syncwarp();
+            sorted = idx + s;
+        } else {
+            int N = 2;
+            while (N < m) N <<= 1;
+            for (int e = lane; e < N; e += 32) {
+                if (e < m) {
+                    skey[e] = block_key64(droplet_block((uint32_t)(s + e), prm.step, rk));
+                    sid[e] = s + e;
+                } else {
+                    skey[e] = ~0ull;
+                    sid[e] = 0x7fffffff;
+                }
+            }
+            __syncwarp();
+            warp_bitonic(skey, sid, N, lane);
+            if (prm.write_idx)
+                for (int e = lane; e < m; e += 32) idx[s + e] = sid[e];
+        }
+        const double norm = pair_norm(m, prm.dtdv);
+        for (int q = lane; q < (m >> 1); q += 32) {
+            int a = sorted[2 * q], b = sorted[2 * q + 1];
+            double u = block_uniform(droplet_block((uint32_t)a, prm.step, rk));
+            int r = collide_pair_exact(xi, v, a, b, u, norm, prm.kernel, prm.kparam);
+            events += r & 1;
+            zeros += (r >> 1) & 1;
+        }
+        __syncwarp();
+    }
+    events = __reduce_add_sync(0xffffffffu, events);
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    if (lane == 0) {
+        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a7: stable in-place stream compaction of xi == 0 (single pass, decoupled look-back)
+// ---------------------------------------------------------------------------------------------
+// A tile's aggregate is published only after the whole tile sits in shared memory, and a tile
+// learns its output offset only after every earlier tile has published: so by the time a tile
+// writes into the (earlier) storage positions, everything there has been read.  Tiles are handed
+// out in order by a ticket, which guarantees forward progress of the look-back.
+constexpr unsigned long long kFlagAggregate = 1ull << 62, kFlagInclusive = 2ull << 62;
+
+__global__ void __launch_bounds__(kCompactThreads)
+k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
+          unsigned long long *__restrict__ status)
+{
+    __shared__ int64_t s_xi[kCompactTile];
+    __shared__ double s_v[kCompactTile];
+    __shared__ int32_t s_c[kCompactTile];
+    __shared__ int s_warp_cnt[kCompactThreads / 32];
+    __shared__ int s_tile, s_prefix;
+    if (ctrl->zero_count == 0) return;                 // nothing to remove: every CTA leaves
+    const int n = ctrl->n;
+    const int n_tiles = (n + kCompactTile - 1) / kCompactTile;
+    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
+    constexpr int kItems = kCompactTile / kCompactThreads;      // 8
+    constexpr int kWarpSpan = 32 * kItems;                       // 256 consecutive elements per warp
+    while (true) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&ctrl->ticket, 1);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= n_tiles) break;
+        const int base = tile * kCompactTile;
+        const int cnt = min(kCompactTile, n - base);
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            int e = k * kCompactThreads + tid;
+            if (e < cnt) { s_xi[e] = xi[base + e]; s_v[e] = v[base + e]; s_c[e] = cell[base + e]; }
+        }
+        __syncthreads();
+        unsigned masks[kItems];
+        int wtotal = 0;
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            int e = warp * kWarpSpan + k * 32 + lane;
+            bool keep = (e < cnt) && (s_xi[e] != 0);
+            masks[k] = __ballot_sync(0xffffffffu, keep);
+            wtotal += __popc(masks[k]);
+        }
+        if (lane == 0) s_warp_cnt[warp] = wtotal;
+        __syncthreads();
+        int woff = 0, tile_total = 0;
+#pragma unroll
+        for (int w = 0; w < kCompactThreads / 32; ++w) {
+            int cw = s_warp_cnt[w];
+            if (w < warp) woff += cw;
+            tile_total += cw;
+        }
+        if (tid == 0) {
+            int excl = 0;
+            volatile unsigned long long *vs = status;
+            __threadfence();
+            if (tile == 0) {
+                vs[0] = kFlagInclusive | (unsigned long long)tile_total;
+            } else {
+                vs[tile] = kFlagAggregate | (unsigned long long)tile_total;
+                int t = tile - 1;
+                while (true) {
+                    unsigned long long st = vs[t];
+                    if ((st >> 62) == 0) continue;               // predecessor not published yet
+                    excl += (int)(st & 0xffffffffull);
+                    if ((st >> 62) == 2) break;
+                    --t;
+                }
+                vs[tile] = kFlagInclusive | (unsigned long long)(excl + tile_total);
+            }
+            __threadfence();
+            s_prefix = excl;
+            if (tile == n_tiles - 1) ctrl->n_new = excl + tile_total;
+        }
+        __syncthreads();
+        const int prefix = s_prefix;
+        int run = woff;
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            int e = warp * kWarpSpan + k * 32 + lane;
+            if ((masks[k] >> lane) & 1u) {
+                int dst = prefix + run + __popc(masks[k] & ((1u << lane) - 1u));
+                xi[dst] = s_xi[e];
+                v[dst] = s_v[e];
+                cell[dst] = s_c[e];
+            }
+            run += __popc(masks[k]);
+        }
+    }
+}
+
+__global__ void k_compact_finalize(Ctrl *ctrl)
+{
+    if (ctrl->zero_count > 0) ctrl->n = ctrl->n_new;
+    ctrl->zero_count = 0;
+    ctrl->ticket = 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row a8: moments M0 = sum xi (int64), M1 = sum xi v, M2 = sum xi v^2 (fp64)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kMomentThreads)
+k_moments_global(const int64_t *__restrict__ xi, const double *__restrict__ v, Ctrl *ctrl,
+                 int64_t *__restrict__ part0, double *__restrict__ part1, double *__restrict__ part2,
+                 int64_t *__restrict__ m0, double *__restrict__ m1, double *__restrict__ m2)
+{
+    __shared__ int64_t s0[kMomentThreads / 32];
+    __shared__ double s1[kMomentThreads / 32], s2[kMomentThreads / 32];
+    __shared__ bool s_last;
+    const int n = ctrl->n;
+    int64_t a0 = 0;
+    double a1 = 0.0, a2 = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        int64_t x = xi[i];
+        double vol = v[i];
+        double xv = __dmul_rn(__ll2double_rn(x), vol);
+        a0 += x;
+        a1 = __dadd_rn(a1, xv);
+        a2 = __dadd_rn(a2, __dmul_rn(xv, vol));
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        a0 += __shfl_down_sync(0xffffffffu, a0, d);
+        a1 += __shfl_down_sync(0xffffffffu, a1, d);
+        a2 += __shfl_down_sync(0xffffffffu, a2, d);
+    }
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    if (lane == 0) { s0[warp] = a0; s1[warp] = a1; s2[warp] = a2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int64_t b0 = 0;
+        double b1 = 0.0, b2 = 0.0;
+        for (int w = 0; w < kMomentThreads / 32; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
+        part0[blockIdx.x] = b0; part1[blockIdx.x] = b1; part2[blockIdx.x] = b2;
+        __threadfence();
+        unsigned int done = atomicAdd(&ctrl->moment_done, 1u);
+        s_last = (done == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    // the last CTA sums the per-CTA partials in a fixed order: the result is run-to-run deterministic
+    __threadfence();
+    a0 = 0; a1 = 0.0; a2 = 0.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) {
+        a0 += ((volatile int64_t *)part0)[b];
+        a1 += ((volatile double *)part1)[b];
+        a2 += ((volatile double *)part2)[b];
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        a0 += __shfl_down_sync(0xffffffffu, a0, d);
+        a1 += __shfl_down_sync(0xffffffffu, a1, d);
+        a2 += __shfl_down_sync(0xffffffffu, a2, d);
+    }
+    __syncthreads();
+    if (lane == 0) { s0[warp] = a0; s1[warp] = a1; s2[warp] = a2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int64_t b0 = 0;
+        double b1 = 0.0, b2 = 0.0;
+        for (int w = 0; w < kMomentThreads / 32; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
+        *m0 = b0; *m1 = b1; *m2 = b2;
+        ctrl->moment_done = 0;
+    }
+}
+
+__global__ void k_moments_zero(int n_cell, int64_t *__restrict__ m0, double *__restrict__ m1,
+                               double *__restrict__ m2)
+{
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cell; c += gridDim.x * blockDim.x) {
+        m0[c] = 0; m1[c] = 0.0; m2[c] = 0.0;
+    }
+}
+
+// any storage order: atomics per cell (the fp64 sums are then order-dependent in the last bits)
+__global__ void k_moments_cell_atomic(const int64_t *__restrict__ xi, const double *__restrict__ v,
+                                      const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
+                                      int64_t *__restrict__ m0, double *__restrict__ m1,
+                                      double *__restrict__ m2)
+{
+    const int n = ctrl->n;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        int64_t x = xi[i];
+        double vol = v[i];
+        int c = cell[i];
+        double xv = __dmul_rn(__ll2double_rn(x), vol);
+        atomicAdd(reinterpret_cast<unsigned long long *>(&m0[c]), (unsigned long long)x);
+        atomicAdd(&m1[c], xv);
+        atomicAdd(&m2[c], __dmul_rn(xv, vol));
+    }
+}
+
+}  // namespace sdmk

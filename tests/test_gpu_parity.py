@@ -1,0 +1,291 @@
+"""GPU parity: libsdm (through the C ABI binding) against the CPU oracle, element by element, on
+the same seeded inputs.  Bar (BASELINE.json north_star): multiplicities, permutations, cell tables
+and survivor sets bit-exact; volumes <= 1e-12 relative (they are in fact bit-exact by construction,
+and the tests assert equality); moments <= 1e-12 relative, M0 exact."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def sdm_mod():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2101_06318_b200 as m
+    m.load_library()
+    return m
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _make(sdm_mod, w, capacity=None, options=()):
+    s = sdm_mod.SDM(capacity or max(w.n_sd, 1), w.n_cell)
+    for k, val in options:
+        s.set_option(k, val)
+    s.set_state(_dev(w.xi), _dev(w.v), _dev(w.cell_id))
+    return s
+
+
+def _compare_step(s, xi, v, cell, w, step, check_perm=True):
+    """Advance both sides by one [remove_zero; step] and compare everything."""
+    xi, v, cell = oracle.remove_zero(xi, v, cell)
+    n_gpu = s.remove_zero()
+    assert n_gpu == len(xi), f"survivor count differs at step {step}"
+    idx, cs, nev = oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    gxi, gv, gc = (t.cpu().numpy() for t in s.get_state())
+    assert np.array_equal(gc, cell), f"cell ids differ at step {step}"
+    if check_perm:
+        gidx, gcs = (t.cpu().numpy() for t in s.get_permutation(len(xi)))
+        assert np.array_equal(gcs, cs), f"cell_start differs at step {step}"
+        assert np.array_equal(gidx, idx), f"permutation differs at step {step}"
+    assert np.array_equal(gxi, xi), f"multiplicities differ at step {step}"
+    assert np.array_equal(gv, v), (f"volumes differ at step {step}: max rel "
+                                   f"{np.max(np.abs(gv - v) / v):.3e} (bar 1e-12)")
+    return xi, v, cell, nev
+
+
+def _run_parity(sdm_mod, w, steps, options=(), expect_mode=None):
+    s = _make(sdm_mod, w, options=options)
+    if expect_mode is not None:
+        assert s.counters()["mode"] == expect_mode
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    events = 0
+    for step in range(steps):
+        xi, v, cell, nev = _compare_step(s, xi, v, cell, w, step)
+        events += nev
+    cnt = s.counters()
+    assert cnt["events"] == events and cnt["n_sd"] == len(xi)
+    m0, m1, m2 = s.moments_host()
+    o0, o1, o2 = oracle.moments(xi, v)
+    assert m0 == o0 and abs(m1 - o1) <= 1e-12 * o1 and abs(m2 - o2) <= 1e-12 * o2
+    s.close()
+    return events, len(xi)
+
+
+# ---- the six workload shapes at oracle-sized scale ------------------------------------------------
+
+def test_c6_small_multiplicities_fused(sdm_mod):
+    w = workloads.grid_small_multiplicity(32, 32, 32, shuffled=False)
+    events, n_end = _run_parity(sdm_mod, w, 25, expect_mode=1)
+    assert events > 5000 and n_end < w.n_sd          # collisions, caps, splits and removals happened
+
+
+def test_c6_small_multiplicities_general(sdm_mod):
+    w = workloads.grid_small_multiplicity(32, 32, 32, shuffled=True)
+    events, n_end = _run_parity(sdm_mod, w, 25, expect_mode=0)
+    assert events > 5000 and n_end < w.n_sd
+
+
+def test_c6_sorted_state_forced_through_general_path(sdm_mod):
+    w = workloads.grid_small_multiplicity(16, 16, 37, shuffled=False, seed=4)
+    _run_parity(sdm_mod, w, 10, options=[(sdm_mod.OPT_FORCE_GENERAL, 1)], expect_mode=0)
+
+
+def test_c4_poisson_grid_shuffled_and_contiguous(sdm_mod):
+    for shuffled, mode in ((True, 0), (False, 1)):
+        w = workloads.grid_poisson(32, 32, 64.0, shuffled=shuffled, seed=1)
+        w.kparam = 1500.0 * 4000.0   # keep the paper's kernel form, raise b so that events occur in 12 steps
+        events, _ = _run_parity(sdm_mod, w, 12, expect_mode=mode)
+        assert events > 50
+
+
+def test_c1_golovin_box_split_cell(sdm_mod):
+    w = workloads.golovin_box(2 ** 13)
+    events, _ = _run_parity(sdm_mod, w, 40, expect_mode=0)      # one cell of 8192 > 512: bucketed sort
+    assert events > 100
+
+
+def test_c2_golovin_box_2e17_few_steps(sdm_mod):
+    w = workloads.golovin_box(2 ** 17)
+    _run_parity(sdm_mod, w, 3, expect_mode=0)
+
+
+def test_c3_gravitational_box(sdm_mod):
+    w = workloads.gravitational_box(2 ** 14)
+    w.dV = 1e6 / 64                                            # denser box so that events occur early
+    events, _ = _run_parity(sdm_mod, w, 25, expect_mode=0)
+    assert events > 20
+
+
+def test_c5_shape_gravitational_grid_fused(sdm_mod):
+    w = workloads.grid_uniform(16, 16, 256, seed=2)
+    w.dV = 1.0                                                 # p ~ 2.6e-2 per pair instead of 2.6e-5
+    events, _ = _run_parity(sdm_mod, w, 8, expect_mode=1)
+    assert events > 200
+
+
+# ---- ragged, degenerate and maximum-size segments --------------------------------------------------
+
+def _ragged_workload(counts, seed=0, shuffled=False, kparam=0.002):
+    rng = np.random.default_rng(seed)
+    counts = np.asarray(counts)
+    n_cell = len(counts)
+    cell = np.repeat(np.arange(n_cell, dtype=np.int32), counts)
+    n = len(cell)
+    xi = rng.integers(1, 50, n).astype(np.int64)
+    v = rng.uniform(0.5, 2.0, n)
+    if shuffled:
+        p = rng.permutation(n)
+        cell, xi, v = cell[p], xi[p], v[p]
+    return workloads.Workload("ragged", xi, v, np.ascontiguousarray(cell), n_cell, 1.0, 1.0,
+                              workloads.configs.KERNEL_GOLOVIN, kparam, 0, seed=11)
+
+
+@pytest.mark.parametrize("shuffled", [False, True])
+def test_ragged_cells_empty_single_odd_and_cap_sized(sdm_mod, shuffled):
+    counts = [0, 1, 2, 3, 0, 0, 31, 32, 33, 63, 64, 65, 127, 129, 255, 256, 257, 511, 512, 1, 0, 7]
+    w = _ragged_workload(counts, shuffled=shuffled)
+    _run_parity(sdm_mod, w, 6, expect_mode=0 if shuffled else 1)
+
+
+@pytest.mark.parametrize("shuffled", [False, True])
+def test_cell_just_above_the_warp_cap_goes_through_buckets(sdm_mod, shuffled):
+    w = _ragged_workload([513, 5, 1400, 0, 2, 640], seed=3, shuffled=shuffled, kparam=0.0005)
+    _run_parity(sdm_mod, w, 5, expect_mode=0)
+
+
+def test_tiny_segment_cap_exercises_the_counting_fallback(sdm_mod):
+    w = _ragged_workload([40, 3, 0, 90, 17, 200], seed=5, shuffled=True)
+    _run_parity(sdm_mod, w, 4, options=[(sdm_mod.OPT_SEGMENT_CAP, 8)], expect_mode=0)
+    w = _ragged_workload([8, 3, 0, 7, 1, 8], seed=6, shuffled=False)
+    _run_parity(sdm_mod, w, 4, options=[(sdm_mod.OPT_SEGMENT_CAP, 8)], expect_mode=1)
+
+
+def test_empty_and_single_droplet_states(sdm_mod):
+    s = sdm_mod.SDM(16, 3)
+    e64, ef, e32 = (torch.empty(0, dtype=t, device="cuda") for t in (torch.int64, torch.float64, torch.int32))
+    s.set_state(e64, ef, e32)
+    s.coalescence_step(1.0, 1.0, 0, 1.0, 0, 0)
+    idx, cs = s.get_permutation(0)
+    assert cs.cpu().tolist() == [0, 0, 0, 0]
+    assert s.remove_zero() == 0 and s.moments_host() == (0, 0.0, 0.0)
+    with pytest.raises(sdm_mod.SdmError):       # the permutation of a step does not survive compaction
+        s.get_permutation(0)
+    s.set_state(_dev(np.array([7], dtype=np.int64)), _dev(np.array([2.5])), _dev(np.array([1], dtype=np.int32)))
+    s.coalescence_step(1.0, 1.0, 0, 1.0, 0, 0)
+    xi, v, c = s.get_state()
+    assert xi.cpu().tolist() == [7] and v.cpu().tolist() == [2.5]
+    idx, cs = s.get_permutation(1)
+    assert idx.cpu().tolist() == [0] and cs.cpu().tolist() == [0, 0, 1, 1]
+    assert s.moments_host() == (7, 17.5, 43.75)
+    s.close()
+
+
+def test_zero_multiplicities_in_the_input_state(sdm_mod):
+    # DESIGN.md R11: zeros occupy a slot, take part in the permutation, their pairs are no-ops
+    rng = np.random.default_rng(8)
+    for shuffled in (False, True):
+        w = _ragged_workload([50, 64, 9, 130], seed=9, shuffled=shuffled, kparam=0.01)
+        w.xi[rng.random(w.n_sd) < 0.3] = 0
+        s = _make(sdm_mod, w)
+        assert s.counters()["zeros"] == int((w.xi == 0).sum())
+        xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+        idx, cs, _ = oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, 0)
+        s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, 0)
+        gxi, gv, _ = (t.cpu().numpy() for t in s.get_state())
+        gidx, gcs = (t.cpu().numpy() for t in s.get_permutation(w.n_sd))
+        assert np.array_equal(gidx, idx) and np.array_equal(gxi, xi) and np.array_equal(gv, v)
+        for step in range(1, 4):
+            xi, v, cell, _ = _compare_step(s, xi, v, cell, w, step)
+        s.close()
+
+
+def test_compaction_many_tiles_and_all_removed(sdm_mod):
+    rng = np.random.default_rng(12)
+    n = 3 * 2048 * 7 + 123
+    xi = rng.integers(0, 3, n).astype(np.int64)
+    xi[5000:9000] = 0                                   # a fully empty tile
+    v = rng.random(n) + 0.1
+    cell = np.sort(rng.integers(0, 50, n)).astype(np.int32)
+    s = sdm_mod.SDM(n, 50)
+    s.set_state(_dev(xi), _dev(v), _dev(cell))
+    keep = xi != 0
+    assert s.remove_zero() == int(keep.sum())
+    gxi, gv, gc = (t.cpu().numpy() for t in s.get_state())
+    assert np.array_equal(gxi, xi[keep]) and np.array_equal(gv, v[keep]) and np.array_equal(gc, cell[keep])
+    assert s.remove_zero() == int(keep.sum())            # second call: zero-count fast path, no change
+    assert s.counters()["zeros"] == 0
+    s.set_state(_dev(np.zeros(5000, dtype=np.int64)), _dev(np.ones(5000)), _dev(np.zeros(5000, dtype=np.int32)))
+    assert s.remove_zero() == 0
+    s.close()
+
+
+def test_per_cell_moments(sdm_mod):
+    for shuffled in (False, True):
+        w = workloads.grid_poisson(16, 16, 40.0, shuffled=shuffled, seed=3)
+        s = _make(sdm_mod, w)
+        m0, m1, m2 = s.moments_host(per_cell=True)
+        o0, o1, o2 = oracle.moments(w.xi, w.v, w.cell_id, w.n_cell, per_cell=True)
+        assert np.array_equal(m0, o0)
+        assert np.all(np.abs(m1 - o1) <= 1e-12 * o1) and np.all(np.abs(m2 - o2) <= 1e-12 * o2)
+        d0, d1, d2 = s.moments(per_cell=False)
+        g0, g1, g2 = oracle.moments(w.xi, w.v)
+        assert int(d0.cpu()[0]) == g0 and abs(float(d1.cpu()[0]) - g1) <= 1e-12 * g1
+        s.close()
+
+
+def test_validation_and_error_codes(sdm_mod):
+    s = sdm_mod.SDM(8, 2)
+    good = (np.array([1, 2], dtype=np.int64), np.array([1.0, 2.0]), np.array([0, 1], dtype=np.int32))
+    for bad in ((np.array([1, -2], dtype=np.int64), good[1], good[2]),
+                (good[0], np.array([1.0, 0.0]), good[2]),
+                (good[0], np.array([1.0, np.inf]), good[2]),
+                (good[0], np.array([np.nan, 1.0]), good[2]),
+                (good[0], good[1], np.array([0, 2], dtype=np.int32)),
+                (good[0], good[1], np.array([-1, 0], dtype=np.int32))):
+        with pytest.raises(sdm_mod.SdmError) as e:
+            s.set_state(*(_dev(a) for a in bad))
+        assert e.value.code == -1
+        with pytest.raises(sdm_mod.SdmError) as e:
+            s.coalescence_step(1.0, 1.0, 0, 1.0, 0, 0)
+        assert e.value.code == -4
+    s.set_state(*(_dev(a) for a in good))
+    for dt, dV, kern in ((-1.0, 1.0, 0), (1.0, 0.0, 0), (1.0, 1.0, 7), (float("nan"), 1.0, 0)):
+        with pytest.raises(sdm_mod.SdmError) as e:
+            s.coalescence_step(dt, dV, kern, 1.0, 0, 0)
+        assert e.value.code == -1
+    with pytest.raises(sdm_mod.SdmError) as e:
+        s.set_state(_dev(np.ones(9, dtype=np.int64)), _dev(np.ones(9)), _dev(np.zeros(9, dtype=np.int32)))
+    assert e.value.code == -2
+    s.close()
+
+
+def test_run_equals_per_step_calls_and_host_variants(sdm_mod):
+    w = workloads.grid_small_multiplicity(16, 16, 20, shuffled=True, seed=7)
+    a = _make(sdm_mod, w)
+    b = sdm_mod.SDM(w.n_sd, w.n_cell)
+    b.set_state_host(torch.from_numpy(w.xi).pin_memory(), torch.from_numpy(w.v).pin_memory(),
+                     torch.from_numpy(w.cell_id).pin_memory())
+    for step in range(9):
+        a.remove_zero(sync=False)
+        a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 5, step)
+    b.run(w.dt, w.dV, w.kernel, w.kparam, 5, 0, 9, True)
+    hx, hv, hc = (torch.empty(w.n_sd, dtype=t).pin_memory() for t in (torch.int64, torch.float64, torch.int32))
+    n = b.get_state_host(hx, hv, hc)
+    ax, av, ac = (t.cpu() for t in a.get_state())
+    assert n == len(ax) and torch.equal(hx[:n], ax) and torch.equal(hv[:n], av) and torch.equal(hc[:n], ac)
+    a.close(), b.close()
+
+
+def test_results_do_not_depend_on_step_order_of_calls_only_on_seed_and_step(sdm_mod):
+    # the RNG is counter-based: (seed, step) fully determines a step, so a checkpoint is the state
+    w = workloads.grid_small_multiplicity(8, 8, 30, seed=2)
+    a = _make(sdm_mod, w)
+    a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 1, 17)
+    x1 = a.get_state()[0].clone()
+    a.set_state(_dev(w.xi), _dev(w.v), _dev(w.cell_id))
+    a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 1, 17)
+    assert torch.equal(x1, a.get_state()[0])
+    a.set_state(_dev(w.xi), _dev(w.v), _dev(w.cell_id))
+    a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 1, 18)
+    assert not torch.equal(x1, a.get_state()[0])
+    a.close()
