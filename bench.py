@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the SDM coalescence hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl reference]
+
+One "step" = one pass of the whole hot path (rows a1-a8 of DESIGN.md) over the resident state:
+    sdm_remove_zero -> sdm_coalescence_step -> sdm_moments (global).
+Default workload: C5 of BASELINE.json (512x512 cells x 256 droplets = 2^26 super-droplets,
+gravitational kernel), the configuration the >= 60 % HBM-roofline target is quoted on; it is 1.25 GiB
+of state, far larger than the 126 MB L2, so no L2 flush is needed between iterations.
+
+Prints ONE JSON line (rank 0).  N > 1 (under torchrun): every rank runs its own shard of cells on
+its own GPU -- cells are independent, there is no data-path collective -- weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "super-droplet-steps/s"
+UNIT = "sd-steps/s"
+
+# algorithmic bytes per droplet-step: compulsory traffic of the method
+B_ALG_FUSED_KERNEL = 20.0      # read xi 8 + v 8, write idx 4 (dominant kernel, cell-contiguous path)
+B_ALG_CELL_INDEX = 4.0         # read cell_id
+B_ALG_MOMENTS = 16.0           # read xi, v
+B_ALG_STEP = B_ALG_FUSED_KERNEL + B_ALG_CELL_INDEX + B_ALG_MOMENTS   # remove_zero: 0 when nothing to remove
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def build_workload(name: str, rank: int = 0, scale_cells: int | None = None):
+    import workloads
+    if name == "C5":
+        nx = ny = scale_cells or 512
+        return workloads.grid_uniform(nx, ny, 256, seed=rank), f"C5: {nx}x{ny} cells x 256 droplets, gravitational kernel, cell-contiguous"
+    if name == "C4":
+        return workloads.grid_poisson(shuffled=False, seed=rank), "C4: 128x128 cells, Poisson(64)/cell, Golovin, cell-contiguous"
+    if name == "C4s":
+        return workloads.grid_poisson(shuffled=True, seed=rank), "C4: 128x128 cells, Poisson(64)/cell, Golovin, shuffled storage"
+    if name == "C1":
+        return workloads.golovin_box(2 ** 13), "C1: Golovin box n=2^13"
+    if name == "C2a":
+        return workloads.golovin_box(2 ** 17), "C2: Golovin box n=2^17"
+    if name == "C2b":
+        return workloads.golovin_box(2 ** 20), "C2: Golovin box n=2^20"
+    if name == "C3":
+        return workloads.gravitational_box(2 ** 20), "C3: gravitational box n=2^20"
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            parts = [x.strip() for x in r.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_rate(target_s: float = 12.0):
+    """The oracle as it stands, one thread, on a bounded C5-shaped sample (64x64 cells x 256)."""
+    import oracle
+    import workloads
+    w = workloads.grid_uniform(64, 64, 256, seed=0)
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    steps, t0 = 0, time.perf_counter()
+    while True:
+        xi, v, cell = oracle.remove_zero(xi, v, cell)
+        oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, steps, want_perm=True)
+        oracle.moments(xi, v)
+        steps += 1
+        el = time.perf_counter() - t0
+        if el >= target_s or steps >= 200:
+            break
+    return w.n_sd * steps / el, steps, w.n_sd, el
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores (bounded sample per step)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    import workloads
+    w = workloads.grid_uniform(64, 64, 256, seed=0)
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+
+    def one(step):
+        nonlocal xi, v, cell
+        xi, v, cell = oracle.remove_zero(xi, v, cell)
+        oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+        oracle.moments(xi, v)
+
+    for s in range(args.warmup):
+        one(s)
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        one(args.warmup + s)
+    el = time.perf_counter() - t0
+    value = w.n_sd * args.steps / el
+    sample = "C5-shaped sample: 64x64 cells x 256 droplets (2^20) per step, single thread"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C5: 512x512 cells x 256 droplets, gravitational kernel (reference arm runs a bounded sample)",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="sdm", choices=["sdm", "reference"])
+    ap.add_argument("--workload", default="C5")
+    ap.add_argument("--cells", type=int, default=None, help="C5 only: grid edge (default 512)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import paper_2101_06318_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libsdm has no CPU fallback")
+    pkg.load_library()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w, wname = build_workload(args.workload, rank, args.cells)
+    dev = torch.device("cuda", local)
+    s = pkg.SDM(w.n_sd, w.n_cell, device=dev)
+    hx = torch.from_numpy(w.xi).pin_memory()
+    hv = torch.from_numpy(w.v).pin_memory()
+    hc = torch.from_numpy(w.cell_id).pin_memory()
+    s.set_state_host(hx, hv, hc)
+    s.set_option(pkg.OPT_TIMING, 1)
+    mode = s.counters()["mode"]
+    mom = s.moments()
+
+    def one_step(step):
+        s.remove_zero(sync=False)
+        s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+        s.moments(out=mom)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for st in range(args.warmup):
+        one_step(st)
+    barrier()
+    s.timing()                                   # drop warm-up kernel timings
+    launches0 = s.counters()["launches"]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for st in range(args.steps):
+        one_step(args.warmup + st)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = ev0.elapsed_time(ev1)
+    kernel_ms, kernel_n = s.timing()
+    cnt = s.counters()
+    launches = cnt["launches"] - launches0
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * w.n_sd * args.steps / (ms * 1e-3)
+
+    # end to end through the C ABI with HOST buffers: H2D of the state, the step, D2H of the state
+    e2e = None
+    if not args.no_e2e:
+        ox = torch.empty(w.n_sd, dtype=torch.int64).pin_memory()
+        ov = torch.empty(w.n_sd, dtype=torch.float64).pin_memory()
+        oc = torch.empty(w.n_sd, dtype=torch.int32).pin_memory()
+
+        def e2e_step(step):
+            s.set_state_host(hx, hv, hc)
+            one_step(step)
+            return s.get_state_host(ox, ov, oc)
+
+        e2e_step(0)
+        barrier()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for st in range(args.e2e_steps):
+            e2e_step(1 + st)
+        e1.record()
+        barrier()
+        wall = time.perf_counter() - t0
+        ems = max(e0.elapsed_time(e1), wall * 1e3)
+        if dist is not None:
+            t = torch.tensor([ems], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        e2e = {"value": world * w.n_sd * args.e2e_steps / (ems * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": 20 * w.n_sd, "d2h_bytes_per_step": 20 * w.n_sd + 8,
+               "steps": args.e2e_steps, "ms_per_step": ems / args.e2e_steps,
+               "what": "sdm_set_state_host + remove_zero + coalescence_step + moments + sdm_get_state_host, pinned host buffers"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peak_gbs()
+    roofline = None
+    if kernel_n > 0:
+        per_launch_s = kernel_ms * 1e-3 / kernel_n
+        b_alg = B_ALG_FUSED_KERNEL if mode == 1 else None
+        if b_alg is not None:
+            achieved = b_alg * w.n_sd / per_launch_s / 1e9
+            roofline = {"bound": "hbm", "kernel": "k_fused_cells (per-cell sort + pairs + update)",
+                        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                        "traffic": None, "peak_source": peak_src, "ms_per_launch": per_launch_s * 1e3,
+                        "launches_timed": kernel_n, "alg_bytes_per_droplet": b_alg,
+                        "kernel_share_of_step": kernel_ms / ms if ms > 0 else None,
+                        "whole_step": {"alg_bytes_per_droplet": B_ALG_STEP,
+                                       "achieved": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9,
+                                       "frac": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9 / peak}}
+        else:
+            roofline = {"bound": "hbm", "kernel": "k_segment_sort (general path; L2-resident workload)",
+                        "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
+                        "ms_per_launch": per_launch_s * 1e3, "launches_timed": kernel_n}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic_fused_kernel.json")
+    if roofline is not None and mode == 1 and os.path.exists(traffic_file):
+        try:
+            with open(traffic_file) as f:
+                tf = json.load(f)
+            if tf.get("n_sd") == w.n_sd:
+                roofline["traffic"] = tf.get("dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        rate, osteps, on, oel = oracle_sample_rate()
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"C5-shaped sample: 64x64 cells x 256 droplets (n_sd={on}), {osteps} steps in {oel:.1f} s, single thread"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "n_sd_per_gpu": w.n_sd, "n_cell_per_gpu": w.n_cell,
+                   "step": "sdm_remove_zero + sdm_coalescence_step + sdm_moments(global)",
+                   "path": "fused cell-contiguous" if mode == 1 else "general",
+                   "l2": "inputs larger than L2 (no flush)" if 20 * w.n_sd > 2 * 126e6 else "L2-resident workload (no flush; latency/launch-bound)",
+                   "parallelism": f"cells sharded over {world} GPU(s), no data-path collective"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "events_in_run": cnt["events"],
+    }
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

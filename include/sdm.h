@@ -50,7 +50,8 @@ enum {
     SDM_OPT_FORCE_GENERAL = 1, /* [0] 1: never take the cell-contiguous fused path                 */
     SDM_OPT_SEGMENT_CAP = 2,   /* [0] >0: override the largest segment a warp sorts on chip (tests) */
     SDM_OPT_WRITE_IDX = 3,     /* [1] 0: do not export the permutation (idx is then undefined)      */
-    SDM_OPT_SCREENING = 4      /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
+    SDM_OPT_SCREENING = 4,     /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
+    SDM_OPT_TIMING = 5         /* [0] 1: bracket the dominant kernel of each step with CUDA events   */
 };
 
 /* Counter slots returned by sdm_get_counters. */
@@ -133,6 +134,12 @@ int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t
 
 /* Reads SDM_CNT_COUNT counters into counters_host.  SYNCHRONOUS. */
 int sdm_get_counters(sdm_t *h, int64_t *counters_host);
+
+/* With SDM_OPT_TIMING on: synchronises, sums the CUDA-event durations [ms] recorded around the
+ * dominant kernel of each coalescence step since the last call (the fused per-cell kernel on the
+ * cell-contiguous path, the segment-sort kernel on the general path), returns their number, and
+ * clears the record.  At most 4096 launches are recorded between two calls. */
+int sdm_get_timing(sdm_t *h, double *total_ms, int64_t *n_launches);
 
 /* Message for the last error on this handle (never NULL; "" if none).  h may be NULL: then the
  * message of the last failed sdm_create on this thread. */

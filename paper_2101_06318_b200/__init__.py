@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     OPT_SEGMENT_CAP,
     OPT_WRITE_IDX,
     OPT_SCREENING,
+    OPT_TIMING,
     load_library,
     library_path,
     workspace_bytes,

@@ -16,6 +16,7 @@ OPT_FORCE_GENERAL = 1
 OPT_SEGMENT_CAP = 2
 OPT_WRITE_IDX = 3
 OPT_SCREENING = 4
+OPT_TIMING = 5
 CNT_NAMES = ("n_sd", "events", "zeros", "launches", "mode", "max_cell", "exact_evals", "reserved")
 
 SDM_OK, SDM_EINVAL, SDM_ECAPACITY, SDM_ECUDA, SDM_ESTATE = 0, -1, -2, -3, -4
@@ -26,7 +27,7 @@ SYMBOLS = (
     "sdm_version", "sdm_workspace_bytes", "sdm_create", "sdm_destroy", "sdm_set_option",
     "sdm_set_state", "sdm_set_state_host", "sdm_get_state", "sdm_get_state_host",
     "sdm_coalescence_step", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
-    "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_last_error",
+    "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
 )
 
 
@@ -75,6 +76,7 @@ def load_library() -> C.CDLL:
     L.sdm_get_permutation.argtypes = [vp, vp, vp]
     L.sdm_run.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64, i64, C.c_int]
     L.sdm_get_counters.argtypes = [vp, C.POINTER(i64)]
+    L.sdm_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
     L.sdm_last_error.argtypes = [vp]
     L.sdm_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -235,6 +237,12 @@ class SDM:
         k = _kernel(kernel, kparam)
         self._check(self._lib.sdm_run(self._h, float(dt), float(dV), C.byref(k), int(seed), int(step0),
                                       int(n_steps), 1 if remove_zero_each_step else 0))
+
+    def timing(self):
+        """(total_ms, n_launches) of the dominant kernel since the last call (needs OPT_TIMING)."""
+        ms, cnt = C.c_double(0.0), C.c_int64(0)
+        self._check(self._lib.sdm_get_timing(self._h, C.byref(ms), C.byref(cnt)))
+        return ms.value, cnt.value
 
     def counters(self) -> dict:
         arr = (C.c_int64 * 8)()

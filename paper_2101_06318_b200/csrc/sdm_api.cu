@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -92,6 +93,9 @@ struct sdm {
     int seg_cap = kWarpCap;
     bool write_idx = true;
     bool screening = true;
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
+    size_t ev_used = 0;
     int64_t launches = 0;
     std::string err;
 };
@@ -121,6 +125,31 @@ int cuda_fail(sdm_t *h, cudaError_t e, const char *what)
         (h)->launches += 1;                                                   \
         cudaError_t e_ = cudaGetLastError();                                  \
         if (e_ != cudaSuccess) return cuda_fail((h), e_, "launch " #kernel);  \
+    } while (0)
+
+constexpr size_t kMaxTimedLaunches = 4096;
+
+// CUDA-event bracket around the dominant kernel (SDM_OPT_TIMING)
+int timing_mark(sdm_t *h)
+{
+    if (!h->timing || h->ev_used >= 2 * kMaxTimedLaunches) return SDM_OK;
+    if (h->ev_used >= h->ev.size()) {
+        cudaEvent_t e;
+        SDM_CUDA(h, cudaEventCreate(&e));
+        h->ev.push_back(e);
+    }
+    SDM_CUDA(h, cudaEventRecord(h->ev[h->ev_used], h->stream));
+    h->ev_used += 1;
+    return SDM_OK;
+}
+
+#define SDM_TIMED(h, stmt)                                 \
+    do {                                                   \
+        int rc_ = timing_mark(h);                          \
+        if (rc_ != SDM_OK) return rc_;                     \
+        stmt;                                              \
+        rc_ = timing_mark(h);                              \
+        if (rc_ != SDM_OK) return rc_;                     \
     } while (0)
 
 inline int grid_for(const sdm_t *h, int64_t work, int block, int per_sm)
@@ -176,9 +205,9 @@ int enqueue_step(sdm_t *h, const StepParams &prm)
     if (use_fused(h)) {
         SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, n_ub, 256, 16), 256, 0, h->cell, h->ctrl, h->n_cell,
                    h->cell_start);
-        SDM_LAUNCH(h, k_fused_cells_v1, grid_for(h, (int64_t)h->n_cell * 32, kSortWarps * 32, 4),
-                   kSortWarps * 32, kSortSmem, h->xi, h->v, h->cell_start, h->n_cell, h->seg_cap, h->idx,
-                   h->ctrl, prm);
+        SDM_TIMED(h, SDM_LAUNCH(h, k_fused_cells_v1, grid_for(h, (int64_t)h->n_cell * 32, kSortWarps * 32, 4),
+                                kSortWarps * 32, kSortSmem, h->xi, h->v, h->cell_start, h->n_cell, h->seg_cap,
+                                h->idx, h->ctrl, prm));
         return SDM_OK;
     }
     const bool split = h->max_count > h->seg_cap;
@@ -205,8 +234,9 @@ int enqueue_step(sdm_t *h, const StepParams &prm)
     SDM_LAUNCH(h, k_scatter, g, 256, 0, h->cell, h->ctrl, split ? 1 : 0, h->cell_bits, h->bucket_base,
                seg_start, cursor, h->order, prm.seed, prm.step);
     int64_t seg_ub = split ? h->L.nb_max : (int64_t)h->n_cell;
-    SDM_LAUNCH(h, k_segment_sort, grid_for(h, seg_ub * 32, kSortWarps * 32, 4), kSortWarps * 32, kSortSmem,
-               seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed, prm.step);
+    SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort, grid_for(h, seg_ub * 32, kSortWarps * 32, 4), kSortWarps * 32,
+                            kSortSmem, seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed,
+                            prm.step));
     SDM_LAUNCH(h, k_pairs_by_position, g, 256, 0, h->xi, h->v, h->cell, h->idx, h->cell_start, h->ctrl, prm);
     return SDM_OK;
 }
@@ -348,6 +378,7 @@ int sdm_destroy(sdm_t *h)
     if (!h) return SDM_EINVAL;
     cudaStreamSynchronize(h->stream);
     if (h->ctrl_host) cudaFreeHost(h->ctrl_host);
+    for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
     delete h;
     return SDM_OK;
 }
@@ -366,6 +397,7 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         return SDM_OK;
     case SDM_OPT_WRITE_IDX: h->write_idx = value != 0; return SDM_OK;
     case SDM_OPT_SCREENING: h->screening = value != 0; return SDM_OK;
+    case SDM_OPT_TIMING: h->timing = value != 0; h->ev_used = 0; return SDM_OK;
     default: return fail(h, SDM_EINVAL, "unknown option");
     }
 }
@@ -533,6 +565,24 @@ int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t
         if (rc != SDM_OK) return rc;
         h->stepped = true;
     }
+    return SDM_OK;
+}
+
+int sdm_get_timing(sdm_t *h, double *total_ms, int64_t *n_launches)
+{
+    if (!h || !total_ms || !n_launches) return SDM_EINVAL;
+    SDM_CUDA(h, cudaStreamSynchronize(h->stream));
+    double total = 0.0;
+    int64_t count = 0;
+    for (size_t i = 0; i + 1 < h->ev_used; i += 2) {
+        float ms = 0.0f;
+        SDM_CUDA(h, cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
+        total += ms;
+        count += 1;
+    }
+    h->ev_used = 0;
+    *total_ms = total;
+    *n_launches = count;
     return SDM_OK;
 }
 
