@@ -14,6 +14,7 @@
 #include <math_constants.h>
 
 #include "sdm_kernels.cuh"
+#include "sdm_fused.cuh"
 
 using namespace sdmk;
 
@@ -163,7 +164,7 @@ inline int grid_for(const sdm_t *h, int64_t work, int block, int per_sm)
 
 bool use_fused(const sdm_t *h)
 {
-    return h->sorted && !h->force_general && h->max_count <= h->seg_cap;
+    return h->sorted && !h->force_general && h->max_count <= h->seg_cap && h->max_count <= 512;
 }
 
 constexpr size_t kSortSmem = (size_t)kSortWarps * kWarpCap * (sizeof(uint64_t) + sizeof(int));
@@ -193,7 +194,7 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.write_idx = h->write_idx ? 1 : 0;
     prm.seed = seed;
     prm.step = step;
-    prm.screening = 0;
+    prm.screening = h->screening ? 1 : 0;
     prm.scr_c = 0.0f;
     return SDM_OK;
 }
@@ -205,9 +206,15 @@ int enqueue_step(sdm_t *h, const StepParams &prm)
     if (use_fused(h)) {
         SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, n_ub, 256, 16), 256, 0, h->cell, h->ctrl, h->n_cell,
                    h->cell_start);
-        SDM_TIMED(h, SDM_LAUNCH(h, k_fused_cells_v1, grid_for(h, (int64_t)h->n_cell * 32, kSortWarps * 32, 4),
-                                kSortWarps * 32, kSortSmem, h->xi, h->v, h->cell_start, h->n_cell, h->seg_cap,
-                                h->idx, h->ctrl, prm));
+        const int gf = grid_for(h, (int64_t)h->n_cell * 32, kFusedWarps * 32, 8);
+#define SDM_FUSED(EE)                                                                                   \
+    SDM_TIMED(h, SDM_LAUNCH(h, k_fused_cells<EE>, gf, kFusedWarps * 32, 0, h->xi, h->v, h->cell_start,   \
+                            h->n_cell, h->idx, h->ctrl, prm))
+        if (h->max_count <= 64) SDM_FUSED(2);
+        else if (h->max_count <= 128) SDM_FUSED(4);
+        else if (h->max_count <= 256) SDM_FUSED(8);
+        else SDM_FUSED(16);
+#undef SDM_FUSED
         return SDM_OK;
     }
     const bool split = h->max_count > h->seg_cap;
@@ -361,8 +368,6 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
     e = cudaFuncSetAttribute(k_segment_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort)");
-    e = cudaFuncSetAttribute(k_fused_cells_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_v1)");
     e = cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(ctrl)");
     e = cudaMemsetAsync(h->cell_start, 0, ((size_t)n_cell + 1) * 4, h->stream);

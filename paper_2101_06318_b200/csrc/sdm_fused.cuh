@@ -1,0 +1,316 @@
+// sdm_fused.cuh -- the dominant kernel: one SDM coalescence step on cell-contiguous storage.
+//
+// One warp owns one cell (E droplets per lane, cell capacity N = 32*E).  Per cell:
+//   1. stream xi, v once (coalesced, evict-first) and reduce an upper bound of the largest
+//      multiplicity and volume of the cell -> P_cell, an upper bound of Eq. 3 for EVERY pair the
+//      permutation could form in this cell ("screening", below);
+//   2. one Philox4x32-10 block per droplet (row a1) -> a packed 32-bit sort word
+//      (top key bits | local index) and a flag "this droplet, as first-in-pair, could fire";
+//   3. register-resident bitonic network over the 32*E packed words: in-lane min/max for strides
+//      < E, __shfl_xor for lane strides (row a3); words that tie on the truncated key are put in
+//      exact (key64, storage index) order by a rare warp-uniform slow path, so idx is bit-exact;
+//   4. idx written as vectors (row a3 output); pairs (2m, 2m+1) sit in one lane (row a4);
+//   5. only pairs whose first member is flagged evaluate Eq. 3-6 in fp64 (rows a5-a6), exactly as
+//      collide_pair_exact does for every pair on the general path.
+//
+// Screening keeps results bit-identical: gamma = floor(p) + [u < p - floor(p)] is 0 whenever
+// p < 1 and u >= p.  P_cell >= p holds for every pair of the cell because K is bounded through the
+// monotone bounds R >= r_j and W >= w_j (gravitational) or 2*v_max (Golovin) with explicit
+// relative margins (1e-4 .. 1e-6) that dwarf all rounding errors of the exact evaluation, and
+// u >= (top 32 bits of u) * 2^-32.  A droplet is flagged iff its top-32-bit uniform <= ceil(P_cell*2^32);
+// P_cell >= 1 (or NaN/inf) flags everything.  Unflagged pairs are skipped: they are no-ops.
+#pragma once
+
+#include "sdm_kernels.cuh"
+
+namespace sdmk {
+
+constexpr int kFusedWarps = 8;
+
+template <int E>
+__device__ __forceinline__ void warp_sort_packed(uint32_t (&x)[E], int lane)
+{
+    constexpr int N = 32 * E;
+#pragma unroll
+    for (int k = 2; k <= N; k <<= 1) {
+        // first stage of the merge: partner p ^ (k-1), minimum to the lower position
+        if (k <= E) {
+#pragma unroll
+            for (int r = 0; r < E; ++r) {
+                const int q = r ^ (k - 1);
+                if (q > r) {
+                    uint32_t lo = min(x[r], x[q]), hi = max(x[r], x[q]);
+                    x[r] = lo; x[q] = hi;
+                }
+            }
+        } else {
+            const int lm = k / E - 1;
+            const bool lower = (lane & (k / (2 * E))) == 0;
+            uint32_t y[E];
+#pragma unroll
+            for (int r = 0; r < E; ++r) y[r] = __shfl_xor_sync(0xffffffffu, x[E - 1 - r], lm);
+#pragma unroll
+            for (int r = 0; r < E; ++r) x[r] = lower ? min(x[r], y[r]) : max(x[r], y[r]);
+        }
+        // remaining stages: partner p ^ j
+#pragma unroll
+        for (int j = k >> 2; j > 0; j >>= 1) {
+            if (j < E) {
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    if ((r & j) == 0) {
+                        uint32_t lo = min(x[r], x[r | j]), hi = max(x[r], x[r | j]);
+                        x[r] = lo; x[r | j] = hi;
+                    }
+                }
+            } else {
+                const int lm = j / E;
+                const bool lower = (lane & lm) == 0;
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    uint32_t y = __shfl_xor_sync(0xffffffffu, x[r], lm);
+                    x[r] = lower ? min(x[r], y) : max(x[r], y);
+                }
+            }
+        }
+    }
+}
+
+// Upper bound of Eq. 3 over all pairs of a cell (see the header of this file).
+__device__ __forceinline__ double cell_probability_bound(int32_t ktype, double kparam, double v_ub,
+                                                         double xi_ub, double norm)
+{
+    double K;
+    if (ktype == 0) {
+        K = kparam * 2.0 * v_ub;                                        // b (v_j + v_k) <= 2 b v_max
+    } else {
+        const double c = 0x1.e8ec8a4aeacc4p-3, pi = 0x1.921fb54442d18p+1;
+        float x32 = __double2float_ru(v_ub * c * 1.000001);
+        double R = (double)cbrtf(x32) * 1.0001;                         // cbrtf: <= 1 ulp (fp32)
+        R = fmax(R, 1e-12);                                             // raising a bound keeps it a bound
+        double W = terminal_velocity(R) * 1.000001;                     // w is non-decreasing in r
+        K = kparam * pi * 4.0 * R * R * W;                              // (r_j + r_k)^2 |w_j - w_k| <= 4 R^2 W
+    }
+    return K * xi_ub * norm * 1.000001;
+}
+
+__device__ __forceinline__ uint32_t flag_threshold(double P)
+{
+    double t = P * 4294967296.0;
+    if (!(t < 4294967295.0)) return 0xFFFFFFFFu;                        // P >= 1, inf or NaN: flag all
+    return (uint32_t)t + 1u;
+}
+
+// Rare: some adjacent sorted words tie on the truncated key.  Re-rank every tie run by the exact
+// (key64, local index) order.  sk: the N sorted words in warp-private shared memory (in/out).
+// Works on shared memory only, so that the caller's register arrays never get their address taken.
+__device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int s, int n_s, int lane, uint64_t seed,
+                                          uint64_t step)
+{
+    const uint32_t N = 32u * (uint32_t)E;
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    // pass 1: new position of each of this lane's words (kept in the upper half of the scratch)
+    uint32_t *np = sk + N;
+    for (int r = 0; r < E; ++r) {
+        const int p = lane * E + r;
+        np[p] = (uint32_t)p;
+        if (p >= n_s) continue;
+        const uint32_t me = sk[p];
+        int a = p, b = p + 1;
+        while (a > 0 && ((sk[a - 1] ^ me) < N)) --a;
+        while (b < n_s && ((sk[b] ^ me) < N)) ++b;
+        if (b - a < 2) continue;
+        const int l = (int)(me & (N - 1));
+        const uint64_t key = block_key64(droplet_block((uint32_t)(s + l), step, rk));
+        int rank = 0;
+        for (int q = a; q < b; ++q) {
+            if (q == p) continue;
+            const int l2 = (int)(sk[q] & (N - 1));
+            const uint64_t key2 = block_key64(droplet_block((uint32_t)(s + l2), step, rk));
+            rank += key_less(key2, l2, key, l) ? 1 : 0;
+        }
+        np[p] = (uint32_t)(a + rank);
+    }
+    __syncwarp();
+    // pass 2: permute (read everything first, then write)
+    uint32_t mine[16], dst[16];
+    for (int r = 0; r < E; ++r) { mine[r] = sk[lane * E + r]; dst[r] = np[lane * E + r]; }
+    __syncwarp();
+    for (int r = 0; r < E; ++r) sk[dst[r]] = mine[r];
+    __syncwarp();
+}
+
+// Rare: the cell has flagged droplets.  Evaluate rows a5-a6 exactly for the pairs they lead.
+// sk: sorted words, sflag: one ballot word per element slot k (bit = lane), both in shared memory.
+__device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int64_t *xi,
+                                            double *v, int s, int n_s, int lane, double dtdv, int32_t ktype,
+                                            double kparam, uint64_t seed, uint64_t step)
+{
+    const uint32_t N = 32u * (uint32_t)E;
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    const double norm = pair_norm(n_s, dtdv);
+    int packed = 0;                                   // events | zeros << 10 | exact << 20
+    for (int m = 0; m < E / 2; ++m) {
+        const int p = lane * E + 2 * m;
+        if (p + 1 >= n_s) continue;
+        const int a = (int)(sk[p] & (N - 1)), b = (int)(sk[p + 1] & (N - 1));
+        if (((sflag[a >> 5] >> (a & 31)) & 1u) == 0) continue;
+        const double u = block_uniform(droplet_block((uint32_t)(s + a), step, rk));
+        const int r = collide_pair_exact(xi, v, s + a, s + b, u, norm, ktype, kparam);
+        packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
+    }
+    return packed;
+}
+
+// Cells larger than the kernel's capacity cannot reach it (the host checks the largest cell at
+// sdm_set_state and cells never grow); this keeps the result defined anyway.
+__device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
+                                          double dtdv, int32_t ktype, double kparam, uint64_t seed,
+                                          uint64_t step)
+{
+    PhiloxKey rk;
+    philox_round_keys(seed, rk);
+    warp_rank_by_counting(nullptr, s, n_s, s, idx, step, rk, lane);
+    __syncwarp();
+    const double norm = pair_norm(n_s, dtdv);
+    int packed = 0;
+    for (int q = lane; q < (n_s >> 1); q += 32) {
+        int a = idx[s + 2 * q], b = idx[s + 2 * q + 1];
+        double u = block_uniform(droplet_block((uint32_t)a, step, rk));
+        int r = collide_pair_exact(xi, v, a, b, u, norm, ktype, kparam);
+        packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
+    }
+    return packed;
+}
+
+template <int E>
+__global__ void __launch_bounds__(kFusedWarps * 32)
+k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
+              int n_cell, int *__restrict__ idx, Ctrl *ctrl, StepParams prm)
+{
+    constexpr int N = 32 * E;
+    static_assert(E >= 2 && (E & (E - 1)) == 0, "E must be an even power of two");
+    __shared__ uint32_t s_scratch[kFusedWarps][2 * N];      // rare paths only
+    __shared__ uint32_t s_flags[kFusedWarps][E];
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    PhiloxKey rk;
+    philox_round_keys(prm.seed, rk);
+    int events = 0, zeros = 0, exact = 0;
+    const int warps_total = gridDim.x * kFusedWarps;
+    for (int c = blockIdx.x * kFusedWarps + warp; c < n_cell; c += warps_total) {
+        const int s = cell_start[c];
+        const int n_s = cell_start[c + 1] - s;
+        if (n_s <= 1) {
+            if (n_s == 1 && lane == 0 && prm.write_idx) idx[s] = s;
+            continue;
+        }
+        if (n_s > N) {
+            const int pk = oversize_cell(xi, v, idx, s, n_s, lane, prm.dtdv, prm.kernel, prm.kparam, prm.seed,
+                                         prm.step);
+            events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
+            continue;
+        }
+        // 1. stream the cell once: bounds of max xi and max v (volumes are positive doubles, so the
+        //    high word orders them; multiplicities are rounded up to fp32)
+        uint32_t vhi_max = 0;
+        float xi_max = 0.0f;
+        if (prm.screening) {
+            int64_t lx[E];
+            double lv[E];
+#pragma unroll
+            for (int k = 0; k < E; ++k) {
+                const int e = k * 32 + lane;
+                lx[k] = (e < n_s) ? __ldcs(reinterpret_cast<const long long *>(xi + s + e)) : 0;
+                lv[k] = (e < n_s) ? __ldcs(v + s + e) : 0.0;
+            }
+#pragma unroll
+            for (int k = 0; k < E; ++k) {
+                vhi_max = max(vhi_max, (uint32_t)__double2hiint(lv[k]));
+                xi_max = fmaxf(xi_max, __ll2float_ru(lx[k]));
+            }
+            vhi_max = __reduce_max_sync(0xffffffffu, vhi_max);
+            xi_max = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(xi_max)));
+        }
+        uint32_t thr = 0xFFFFFFFFu;
+        if (prm.screening) {
+            const double v_ub = __hiloint2double((int)(vhi_max + 1u), 0);
+            const double P = cell_probability_bound(prm.kernel, prm.kparam, v_ub, (double)xi_max,
+                                                    pair_norm(n_s, prm.dtdv));
+            thr = flag_threshold(P);
+        }
+        // 2. Philox block per droplet -> packed sort word + flag
+        uint32_t x[E];
+        uint32_t fmask = 0;
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            const int e = k * 32 + lane;
+            const uint4 w = droplet_block((uint32_t)(s + e), prm.step, rk);
+            const bool valid = e < n_s;
+            x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)e) : 0xFFFFFFFFu;
+            fmask |= (valid && (w.w <= thr)) ? (1u << k) : 0u;
+        }
+        // 3. sort, then exact order inside truncated-key ties (rare)
+        warp_sort_packed<E>(x, lane);
+        {
+            bool tie = false;
+#pragma unroll
+            for (int r = 0; r + 1 < E; ++r) tie |= ((x[r] ^ x[r + 1]) < (uint32_t)N);
+            const uint32_t nx = __shfl_down_sync(0xffffffffu, x[0], 1);
+            tie |= (lane < 31) && ((x[E - 1] ^ nx) < (uint32_t)N);
+            if (__any_sync(0xffffffffu, tie)) {
+                uint32_t *sk = s_scratch[warp];
+#pragma unroll
+                for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
+                __syncwarp();
+                fix_key_ties(sk, E, s, n_s, lane, prm.seed, prm.step);
+#pragma unroll
+                for (int r = 0; r < E; ++r) x[r] = sk[lane * E + r];
+                __syncwarp();
+            }
+        }
+        // 4. idx
+        if (prm.write_idx) {
+            const int p0 = lane * E;
+            if (((s & 3) == 0) && (E % 4 == 0) && (p0 + E <= n_s)) {
+#pragma unroll
+                for (int r = 0; r < E; r += 4) {
+                    int4 o = make_int4(s + (int)(x[r] & (N - 1)), s + (int)(x[r + 1] & (N - 1)),
+                                       s + (int)(x[r + 2] & (N - 1)), s + (int)(x[r + 3] & (N - 1)));
+                    __stcs(reinterpret_cast<int4 *>(idx + s + p0 + r), o);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < E; ++r)
+                    if (p0 + r < n_s) idx[s + p0 + r] = s + (int)(x[r] & (N - 1));
+            }
+        }
+        // 5. pairs led by a flagged droplet (rare)
+        if (__any_sync(0xffffffffu, fmask != 0)) {
+#pragma unroll
+            for (int k = 0; k < E; ++k) {
+                const uint32_t word = __ballot_sync(0xffffffffu, (fmask >> k) & 1u);
+                if (lane == k) s_flags[warp][k] = word;
+            }
+            uint32_t *sk = s_scratch[warp];
+#pragma unroll
+            for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
+            __syncwarp();
+            const int pk = collide_flagged(sk, s_flags[warp], E, xi, v, s, n_s, lane, prm.dtdv, prm.kernel,
+                                           prm.kparam, prm.seed, prm.step);
+            events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
+            __syncwarp();
+        }
+    }
+    events = __reduce_add_sync(0xffffffffu, events);
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    exact = __reduce_add_sync(0xffffffffu, exact);
+    if (lane == 0) {
+        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+        if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
+    }
+}
+
+}  // namespace sdmk

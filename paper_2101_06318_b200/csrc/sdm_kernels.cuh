@@ -339,7 +339,7 @@ __global__ void k_pairs_by_position(int64_t *__restrict__ xi, double *__restrict
     PhiloxKey rk;
     philox_round_keys(prm.seed, rk);
     const int n = ctrl->n;
-    int events = 0, zeros = 0;
+    int events = 0, zeros = 0, exact = 0;
     for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
         int a = idx[p];
         int c = cell[a];
@@ -352,12 +352,15 @@ __global__ void k_pairs_by_position(int64_t *__restrict__ xi, double *__restrict
         int r = collide_pair_exact(xi, v, a, b, u, pair_norm(n_s, prm.dtdv), prm.kernel, prm.kparam);
         events += r & 1;
         zeros += (r >> 1) & 1;
+        exact += 1;
     }
     events = __reduce_add_sync(0xffffffffu, events);
     zeros = __reduce_add_sync(0xffffffffu, zeros);
+    exact = __reduce_add_sync(0xffffffffu, exact);
     if (lane_id() == 0) {
         if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
         if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+        if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
     }
 }
 
@@ -379,63 +382,6 @@ __global__ void k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl
         for (int cc = prev + 1; cc <= c; ++cc) cell_start[cc] = i;
         if (i == n - 1)
             for (int cc = c + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
-    }
-}
-
-// v1: one warp per cell, (key64, id) bitonic sort in shared memory, pairs read xi/v from global
-__global__ void __launch_bounds__(kSortWarps * 32)
-k_fused_cells_v1(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
-                 int n_cell, int seg_cap, int *__restrict__ idx, Ctrl *ctrl, StepParams prm)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = lane_id();
-    uint64_t *skey = reinterpret_cast<uint64_t *>(smem_raw) + warp * kWarpCap;
-    int *sid = reinterpret_cast<int *>(smem_raw + kSortWarps * kWarpCap * sizeof(uint64_t)) + warp * kWarpCap;
-    PhiloxKey rk;
-    philox_round_keys(prm.seed, rk);
-    int events = 0, zeros = 0;
-    const int warps_total = gridDim.x * kSortWarps;
-    for (int c = blockIdx.x * kSortWarps + warp; c < n_cell; c += warps_total) {
-        const int s = cell_start[c];
-        const int m = cell_start[c + 1] - s;
-        if (m == 0) continue;
-        const int *sorted = sid;
-        if (m > seg_cap) {   // the host only takes this path when max_count <= seg_cap; kept for safety
-            warp_rank_by_counting(nullptr, s, m, s, idx, prm.step, rk, lane);
-            __syncwarp();
-            sorted = idx + s;
-        } else {
-            int N = 2;
-            while (N < m) N <<= 1;
-            for (int e = lane; e < N; e += 32) {
-                if (e < m) {
-                    skey[e] = block_key64(droplet_block((uint32_t)(s + e), prm.step, rk));
-                    sid[e] = s + e;
-                } else {
-                    skey[e] = ~0ull;
-                    sid[e] = 0x7fffffff;
-                }
-            }
-            __syncwarp();
-            warp_bitonic(skey, sid, N, lane);
-            if (prm.write_idx)
-                for (int e = lane; e < m; e += 32) idx[s + e] = sid[e];
-        }
-        const double norm = pair_norm(m, prm.dtdv);
-        for (int q = lane; q < (m >> 1); q += 32) {
-            int a = sorted[2 * q], b = sorted[2 * q + 1];
-            double u = block_uniform(droplet_block((uint32_t)a, prm.step, rk));
-            int r = collide_pair_exact(xi, v, a, b, u, norm, prm.kernel, prm.kparam);
-            events += r & 1;
-            zeros += (r >> 1) & 1;
-        }
-        __syncwarp();
-    }
-    events = __reduce_add_sync(0xffffffffu, events);
-    zeros = __reduce_add_sync(0xffffffffu, zeros);
-    if (lane == 0) {
-        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
-        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
     }
 }
 
