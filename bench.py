@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl reference]
 
 One "step" = one pass of the whole hot path (rows a1-a8 of DESIGN.md) over the resident state:
-    sdm_remove_zero -> sdm_coalescence_step -> sdm_moments (global).
+    sdm_remove_zero -> sdm_coalescence_step_moments (coalescence step + global moments of the new state).
 Default workload: C5 of BASELINE.json (512x512 cells x 256 droplets = 2^26 super-droplets,
 gravitational kernel), the configuration the >= 60 % HBM-roofline target is quoted on; it is 1.25 GiB
 of state, far larger than the 126 MB L2, so no L2 flush is needed between iterations.
@@ -33,8 +33,7 @@ UNIT = "sd-steps/s"
 # algorithmic bytes per droplet-step: compulsory traffic of the method
 B_ALG_FUSED_KERNEL = 20.0      # read xi 8 + v 8, write idx 4 (dominant kernel, cell-contiguous path)
 B_ALG_CELL_INDEX = 4.0         # read cell_id
-B_ALG_MOMENTS = 16.0           # read xi, v
-B_ALG_STEP = B_ALG_FUSED_KERNEL + B_ALG_CELL_INDEX + B_ALG_MOMENTS   # remove_zero: 0 when nothing to remove
+B_ALG_STEP = B_ALG_FUSED_KERNEL + B_ALG_CELL_INDEX   # moments ride on the same pass; remove_zero: 0 when nothing to remove
 
 
 def measured_peak_gbs():
@@ -215,8 +214,7 @@ def main():
 
     def one_step(step):
         s.remove_zero(sync=False)
-        s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
-        s.moments(out=mom)
+        s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step, out=mom)
 
     def barrier():
         if dist is not None:
@@ -279,7 +277,7 @@ def main():
         e2e = {"value": world * w.n_sd * args.e2e_steps / (ems * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": 20 * w.n_sd, "d2h_bytes_per_step": 20 * w.n_sd + 8,
                "steps": args.e2e_steps, "ms_per_step": ems / args.e2e_steps,
-               "what": "sdm_set_state_host + remove_zero + coalescence_step + moments + sdm_get_state_host, pinned host buffers"}
+               "what": "sdm_set_state_host + remove_zero + coalescence_step_moments + sdm_get_state_host, pinned host buffers"}
 
     if rank != 0:
         if dist is not None:
@@ -326,7 +324,7 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": wname, "n_sd_per_gpu": w.n_sd, "n_cell_per_gpu": w.n_cell,
-                   "step": "sdm_remove_zero + sdm_coalescence_step + sdm_moments(global)",
+                   "step": "sdm_remove_zero + sdm_coalescence_step_moments (step + global moments)",
                    "path": "fused cell-contiguous" if mode == 1 else "general",
                    "l2": "inputs larger than L2 (no flush)" if 20 * w.n_sd > 2 * 126e6 else "L2-resident workload (no flush; latency/launch-bound)",
                    "parallelism": f"cells sharded over {world} GPU(s), no data-path collective"},

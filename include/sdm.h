@@ -109,6 +109,14 @@ int sdm_get_state_host(sdm_t *h, int64_t *n_sd, int64_t *xi_host, double *v_host
 int sdm_coalescence_step(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
                          uint64_t step);
 
+/* sdm_coalescence_step followed by sdm_moments(per_cell = 0) of the post-step state, as one call: on
+ * the cell-contiguous path both come out of the same kernel (the state is streamed once).  The
+ * state after the call is identical to sdm_coalescence_step's; M0 is exact; M1, M2 equal
+ * sdm_moments' up to fp64 summation order (<= 1e-12 relative).  ASYNCHRONOUS. */
+int sdm_coalescence_step_moments(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel,
+                                 uint64_t seed, uint64_t step, int64_t *m0_dev, double *m1_dev,
+                                 double *m2_dev);
+
 /* Step 0 of Fig. 3: removes super-droplets with xi == 0 by a STABLE
  * compaction of (xi, v, cell_id).  n_sd_out == NULL: ASYNCHRONOUS (n_sd stays on the device);
  * otherwise SYNCHRONOUS and *n_sd_out receives the new count. */

@@ -26,7 +26,7 @@ _CODES = {-1: "SDM_EINVAL", -2: "SDM_ECAPACITY", -3: "SDM_ECUDA", -4: "SDM_ESTAT
 SYMBOLS = (
     "sdm_version", "sdm_workspace_bytes", "sdm_create", "sdm_destroy", "sdm_set_option",
     "sdm_set_state", "sdm_set_state_host", "sdm_get_state", "sdm_get_state_host",
-    "sdm_coalescence_step", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
+    "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
 )
 
@@ -45,7 +45,8 @@ _lib = None
 
 
 def library_path() -> str:
-    return os.path.join(HERE, "libsdm.so")
+    """In-tree libsdm.so; SDM_LIBRARY overrides the path (to try an alternative build of the same ABI)."""
+    return os.environ.get("SDM_LIBRARY") or os.path.join(HERE, "libsdm.so")
 
 
 def load_library() -> C.CDLL:
@@ -70,6 +71,7 @@ def load_library() -> C.CDLL:
     L.sdm_get_state.argtypes = [vp, C.POINTER(i64), vp, vp, vp]
     L.sdm_get_state_host.argtypes = [vp, C.POINTER(i64), vp, vp, vp]
     L.sdm_coalescence_step.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64]
+    L.sdm_coalescence_step_moments.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64, vp, vp, vp]
     L.sdm_remove_zero.argtypes = [vp, C.POINTER(i64)]
     L.sdm_moments.argtypes = [vp, C.c_int, vp, vp, vp]
     L.sdm_moments_host.argtypes = [vp, C.c_int, vp, vp, vp]
@@ -193,6 +195,17 @@ class SDM:
     def coalescence_step(self, dt, dV, kernel, kparam, seed, step):
         k = _kernel(kernel, kparam)
         self._check(self._lib.sdm_coalescence_step(self._h, float(dt), float(dV), C.byref(k), int(seed), int(step)))
+
+    def coalescence_step_moments(self, dt, dV, kernel, kparam, seed, step, out=None):
+        """One step plus the global moments of the post-step state (device tensors, asynchronous)."""
+        t = self.torch
+        k = _kernel(kernel, kparam)
+        if out is None:
+            out = (t.empty(1, dtype=t.int64, device=self.device), t.empty(1, dtype=t.float64, device=self.device),
+                   t.empty(1, dtype=t.float64, device=self.device))
+        self._check(self._lib.sdm_coalescence_step_moments(self._h, float(dt), float(dV), C.byref(k), int(seed),
+                                                           int(step), self._p(out[0]), self._p(out[1]), self._p(out[2])))
+        return out
 
     def remove_zero(self, sync: bool = True):
         if not sync:

@@ -200,16 +200,28 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
 }
 
 // Fig. 3 steps 1-3 enqueued on the stream
-int enqueue_step(sdm_t *h, const StepParams &prm)
+int enqueue_moments(sdm_t *h, int per_cell, int64_t *m0, double *m1, double *m2);
+
+// m0/m1/m2 != NULL: also produce the global moments of the post-step state
+int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double *m1 = nullptr,
+                 double *m2 = nullptr)
 {
     const int64_t n_ub = h->n_ub;
     if (use_fused(h)) {
-        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, n_ub, 256, 16), 256, 0, h->cell, h->ctrl, h->n_cell,
+        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 3) / 4, 256, 32), 256, 0, h->cell, h->ctrl, h->n_cell,
                    h->cell_start);
         const int gf = grid_for(h, (int64_t)h->n_cell * 32, kFusedWarps * 32, 8);
-#define SDM_FUSED(EE)                                                                                   \
-    SDM_TIMED(h, SDM_LAUNCH(h, k_fused_cells<EE>, gf, kFusedWarps * 32, 0, h->xi, h->v, h->cell_start,   \
-                            h->n_cell, h->idx, h->ctrl, prm))
+#define SDM_FUSED(EE)                                                                                    \
+    do {                                                                                                 \
+        if (m0)                                                                                          \
+            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, true>), gf, kFusedWarps * 32, 0, h->xi, h->v,   \
+                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,   \
+                                    h->part2, m0, m1, m2));                                              \
+        else                                                                                             \
+            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, false>), gf, kFusedWarps * 32, 0, h->xi, h->v,  \
+                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,   \
+                                    h->part2, m0, m1, m2));                                              \
+    } while (0)
         if (h->max_count <= 64) SDM_FUSED(2);
         else if (h->max_count <= 128) SDM_FUSED(4);
         else if (h->max_count <= 256) SDM_FUSED(8);
@@ -245,6 +257,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm)
                             kSortSmem, seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed,
                             prm.step));
     SDM_LAUNCH(h, k_pairs_by_position, g, 256, 0, h->xi, h->v, h->cell, h->idx, h->cell_start, h->ctrl, prm);
+    if (m0) return enqueue_moments(h, 0, m0, m1, m2);
     return SDM_OK;
 }
 
@@ -474,6 +487,20 @@ int sdm_coalescence_step(sdm_t *h, double dt, double dV, const sdm_kernel_t *ker
     int rc = make_params(h, dt, dV, kernel, seed, step, prm);
     if (rc != SDM_OK) return rc;
     rc = enqueue_step(h, prm);
+    if (rc == SDM_OK) h->stepped = true;
+    return rc;
+}
+
+int sdm_coalescence_step_moments(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
+                                 uint64_t step, int64_t *m0_dev, double *m1_dev, double *m2_dev)
+{
+    if (!h) return SDM_EINVAL;
+    if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
+    if (!m0_dev || !m1_dev || !m2_dev) return fail(h, SDM_EINVAL, "moment output pointer is NULL");
+    StepParams prm;
+    int rc = make_params(h, dt, dV, kernel, seed, step, prm);
+    if (rc != SDM_OK) return rc;
+    rc = enqueue_step(h, prm, m0_dev, m1_dev, m2_dev);
     if (rc == SDM_OK) h->stepped = true;
     return rc;
 }

@@ -25,7 +25,14 @@
 
 namespace sdmk {
 
-constexpr int kFusedWarps = 8;
+#ifndef SDM_FUSED_WARPS
+#define SDM_FUSED_WARPS 8
+#endif
+#ifndef SDM_FUSED_MIN_BLOCKS
+#define SDM_FUSED_MIN_BLOCKS 3
+#endif
+constexpr int kFusedWarps = SDM_FUSED_WARPS;
+constexpr int kFusedMinBlocks = SDM_FUSED_MIN_BLOCKS;
 
 template <int E>
 __device__ __forceinline__ void warp_sort_packed(uint32_t (&x)[E], int lane)
@@ -143,10 +150,27 @@ __device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int s, int n_s, i
 
 // Rare: the cell has flagged droplets.  Evaluate rows a5-a6 exactly for the pairs they lead.
 // sk: sorted words, sflag: one ballot word per element slot k (bit = lane), both in shared memory.
+// One pair's contribution to (M0, M1, M2), products rounded as in k_moments_global.
+__device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v, int a, int b, int64_t &p0,
+                                             double &p1, double &p2)
+{
+    const int64_t xa = xi[a], xb = xi[b];
+    const double va = v[a], vb = v[b];
+    const double ya = __dmul_rn(__ll2double_rn(xa), va), yb = __dmul_rn(__ll2double_rn(xb), vb);
+    p0 = xa + xb;
+    p1 = __dadd_rn(ya, yb);
+    p2 = __dadd_rn(__dmul_rn(ya, va), __dmul_rn(yb, vb));
+}
+
+// delta (may be NULL): three doubles of warp-private shared memory per lane; receives the change of
+// (M0, M1, M2) caused by this lane's events (M0 as a double holding an exact integer < 2^53 is not
+// enough in general, so M0's change is stored as the bit pattern of an int64).
 __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int64_t *xi,
                                             double *v, int s, int n_s, int lane, double dtdv, int32_t ktype,
-                                            double kparam, uint64_t seed, uint64_t step)
+                                            double kparam, uint64_t seed, uint64_t step, double *delta)
 {
+    int64_t d0 = 0;
+    double d1 = 0.0, d2 = 0.0;
     const uint32_t N = 32u * (uint32_t)E;
     PhiloxKey rk;
     philox_round_keys(seed, rk);
@@ -158,8 +182,24 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
         const int a = (int)(sk[p] & (N - 1)), b = (int)(sk[p + 1] & (N - 1));
         if (((sflag[a >> 5] >> (a & 31)) & 1u) == 0) continue;
         const double u = block_uniform(droplet_block((uint32_t)(s + a), step, rk));
+        int64_t o0 = 0;
+        double o1 = 0.0, o2 = 0.0;
+        if (delta) pair_moments(xi, v, s + a, s + b, o0, o1, o2);
         const int r = collide_pair_exact(xi, v, s + a, s + b, u, norm, ktype, kparam);
+        if (delta && (r & 1)) {
+            int64_t n0;
+            double n1, n2;
+            pair_moments(xi, v, s + a, s + b, n0, n1, n2);
+            d0 += n0 - o0;
+            d1 = __dadd_rn(d1, __dsub_rn(n1, o1));
+            d2 = __dadd_rn(d2, __dsub_rn(n2, o2));
+        }
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
+    }
+    if (delta) {
+        delta[0] = __longlong_as_double(d0);
+        delta[1] = d1;
+        delta[2] = d2;
     }
     return packed;
 }
@@ -168,7 +208,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 // sdm_set_state and cells never grow); this keeps the result defined anyway.
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
                                           double dtdv, int32_t ktype, double kparam, uint64_t seed,
-                                          uint64_t step)
+                                          uint64_t step, double *delta)
 {
     PhiloxKey rk;
     philox_round_keys(seed, rk);
@@ -182,18 +222,42 @@ __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int 
         int r = collide_pair_exact(xi, v, a, b, u, norm, ktype, kparam);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
+    if (delta) {                                      // here: the cell's whole post-step contribution
+        __syncwarp();
+        int64_t d0 = 0;
+        double d1 = 0.0, d2 = 0.0;
+        for (int q = lane; q < n_s; q += 32) {
+            const int64_t x = xi[s + q];
+            const double vol = v[s + q];
+            const double xv = __dmul_rn(__ll2double_rn(x), vol);
+            d0 += x;
+            d1 = __dadd_rn(d1, xv);
+            d2 = __dadd_rn(d2, __dmul_rn(xv, vol));
+        }
+        delta[0] = __longlong_as_double(d0);
+        delta[1] = d1;
+        delta[2] = d2;
+    }
     return packed;
 }
 
-template <int E>
-__global__ void __launch_bounds__(kFusedWarps * 32)
+// MOM: also produce the global moments (M0, M1, M2) of the state AFTER the step: the pre-step sums
+// are taken from the values streamed for the screening, and every event adds its exact change.
+template <int E, bool MOM>
+__global__ void __launch_bounds__(kFusedWarps * 32, kFusedMinBlocks)
 k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
-              int n_cell, int *__restrict__ idx, Ctrl *ctrl, StepParams prm)
+              int n_cell, int *__restrict__ idx, Ctrl *ctrl, StepParams prm, int64_t *__restrict__ part0,
+              double *__restrict__ part1, double *__restrict__ part2, int64_t *__restrict__ m0,
+              double *__restrict__ m1, double *__restrict__ m2)
 {
     constexpr int N = 32 * E;
     static_assert(E >= 2 && (E & (E - 1)) == 0, "E must be an even power of two");
     __shared__ uint32_t s_scratch[kFusedWarps][2 * N];      // rare paths only
     __shared__ uint32_t s_flags[kFusedWarps][E];
+    __shared__ double s_delta[MOM ? kFusedWarps * 32 * 3 : 1];
+    double *my_delta = MOM ? &s_delta[(threadIdx.x >> 5) * 96 + (threadIdx.x & 31) * 3] : nullptr;
+    int64_t a0 = 0;
+    double a1 = 0.0, a2 = 0.0;
     const int warp = threadIdx.x >> 5, lane = lane_id();
     PhiloxKey rk;
     philox_round_keys(prm.seed, rk);
@@ -203,32 +267,54 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         const int s = cell_start[c];
         const int n_s = cell_start[c + 1] - s;
         if (n_s <= 1) {
-            if (n_s == 1 && lane == 0 && prm.write_idx) idx[s] = s;
+            if (n_s == 1 && lane == 0) {
+                if (prm.write_idx) idx[s] = s;
+                if (MOM) {
+                    const int64_t x1 = xi[s];
+                    const double v1 = v[s], xv = __dmul_rn(__ll2double_rn(x1), v1);
+                    a0 += x1;
+                    a1 = __dadd_rn(a1, xv);
+                    a2 = __dadd_rn(a2, __dmul_rn(xv, v1));
+                }
+            }
             continue;
         }
         if (n_s > N) {
             const int pk = oversize_cell(xi, v, idx, s, n_s, lane, prm.dtdv, prm.kernel, prm.kparam, prm.seed,
-                                         prm.step);
+                                         prm.step, my_delta);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
+            if (MOM) {
+                a0 += __double_as_longlong(my_delta[0]);
+                a1 = __dadd_rn(a1, my_delta[1]);
+                a2 = __dadd_rn(a2, my_delta[2]);
+            }
             continue;
         }
         // 1. stream the cell once: bounds of max xi and max v (volumes are positive doubles, so the
         //    high word orders them; multiplicities are rounded up to fp32)
         uint32_t vhi_max = 0;
         float xi_max = 0.0f;
-        if (prm.screening) {
+        const int nrem = n_s - lane;                      // droplet k*32+lane exists iff nrem > 32k
+        if (prm.screening || MOM) {
             int64_t lx[E];
             double lv[E];
+            const long long *px = reinterpret_cast<const long long *>(xi + s + lane);
+            const double *pv = v + s + lane;
 #pragma unroll
             for (int k = 0; k < E; ++k) {
-                const int e = k * 32 + lane;
-                lx[k] = (e < n_s) ? __ldcs(reinterpret_cast<const long long *>(xi + s + e)) : 0;
-                lv[k] = (e < n_s) ? __ldcs(v + s + e) : 0.0;
+                lx[k] = (nrem > 32 * k) ? __ldcs(px + 32 * k) : 0;
+                lv[k] = (nrem > 32 * k) ? __ldcs(pv + 32 * k) : 0.0;
             }
 #pragma unroll
             for (int k = 0; k < E; ++k) {
                 vhi_max = max(vhi_max, (uint32_t)__double2hiint(lv[k]));
                 xi_max = fmaxf(xi_max, __ll2float_ru(lx[k]));
+                if (MOM) {                                  // absent droplets were loaded as (0, 0.0)
+                    const double xv = __dmul_rn(__ll2double_rn(lx[k]), lv[k]);
+                    a0 += lx[k];
+                    a1 = __dadd_rn(a1, xv);
+                    a2 = __dadd_rn(a2, __dmul_rn(xv, lv[k]));
+                }
             }
             vhi_max = __reduce_max_sync(0xffffffffu, vhi_max);
             xi_max = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(xi_max)));
@@ -242,24 +328,25 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         }
         // 2. Philox block per droplet -> packed sort word + flag
         uint32_t x[E];
-        uint32_t fmask = 0;
+        uint32_t umin = 0xFFFFFFFFu;                      // smallest top uniform word of this lane's droplets
+        const uint32_t sid0 = (uint32_t)(s + lane);
 #pragma unroll
         for (int k = 0; k < E; ++k) {
-            const int e = k * 32 + lane;
-            const uint4 w = droplet_block((uint32_t)(s + e), prm.step, rk);
-            const bool valid = e < n_s;
-            x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)e) : 0xFFFFFFFFu;
-            fmask |= (valid && (w.w <= thr)) ? (1u << k) : 0u;
+            const uint4 w = droplet_block(sid0 + 32u * k, prm.step, rk);
+            const bool valid = nrem > 32 * k;
+            x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)(lane + 32 * k)) : 0xFFFFFFFFu;
+            umin = min(umin, valid ? w.w : 0xFFFFFFFFu);
         }
         // 3. sort, then exact order inside truncated-key ties (rare)
         warp_sort_packed<E>(x, lane);
         {
-            bool tie = false;
-#pragma unroll
-            for (int r = 0; r + 1 < E; ++r) tie |= ((x[r] ^ x[r + 1]) < (uint32_t)N);
+            // words that share the truncated key differ by less than N (necessary, not sufficient:
+            // the slow path re-checks); sorted ascending, so differences are non-negative
             const uint32_t nx = __shfl_down_sync(0xffffffffu, x[0], 1);
-            tie |= (lane < 31) && ((x[E - 1] ^ nx) < (uint32_t)N);
-            if (__any_sync(0xffffffffu, tie)) {
+            uint32_t dmin = (lane < 31) ? nx - x[E - 1] : 0xFFFFFFFFu;
+#pragma unroll
+            for (int r = 0; r + 1 < E; ++r) dmin = min(dmin, x[r + 1] - x[r]);
+            if (__any_sync(0xffffffffu, dmin < (uint32_t)N)) {
                 uint32_t *sk = s_scratch[warp];
 #pragma unroll
                 for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
@@ -273,7 +360,15 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         // 4. idx
         if (prm.write_idx) {
             const int p0 = lane * E;
-            if (((s & 3) == 0) && (E % 4 == 0) && (p0 + E <= n_s)) {
+            if (((s & (N - 1)) == 0) && (E % 4 == 0) && (p0 + E <= n_s)) {
+                // cell start aligned to the capacity: s + local == s | local
+#pragma unroll
+                for (int r = 0; r < E; r += 4) {
+                    int4 o = make_int4(s | (int)(x[r] & (N - 1)), s | (int)(x[r + 1] & (N - 1)),
+                                       s | (int)(x[r + 2] & (N - 1)), s | (int)(x[r + 3] & (N - 1)));
+                    __stcs(reinterpret_cast<int4 *>(idx + s + p0 + r), o);
+                }
+            } else if (((s & 3) == 0) && (E % 4 == 0) && (p0 + E <= n_s)) {
 #pragma unroll
                 for (int r = 0; r < E; r += 4) {
                     int4 o = make_int4(s + (int)(x[r] & (N - 1)), s + (int)(x[r + 1] & (N - 1)),
@@ -287,10 +382,12 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             }
         }
         // 5. pairs led by a flagged droplet (rare)
-        if (__any_sync(0xffffffffu, fmask != 0)) {
-#pragma unroll
+        if (__any_sync(0xffffffffu, umin <= thr)) {
+            // rare: redo the blocks of this lane's droplets to learn which ones are flagged
+#pragma unroll 1
             for (int k = 0; k < E; ++k) {
-                const uint32_t word = __ballot_sync(0xffffffffu, (fmask >> k) & 1u);
+                const uint4 w = droplet_block(sid0 + 32u * k, prm.step, rk);
+                const uint32_t word = __ballot_sync(0xffffffffu, (nrem > 32 * k) && (w.w <= thr));
                 if (lane == k) s_flags[warp][k] = word;
             }
             uint32_t *sk = s_scratch[warp];
@@ -298,8 +395,13 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
             __syncwarp();
             const int pk = collide_flagged(sk, s_flags[warp], E, xi, v, s, n_s, lane, prm.dtdv, prm.kernel,
-                                           prm.kparam, prm.seed, prm.step);
+                                           prm.kparam, prm.seed, prm.step, my_delta);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
+            if (MOM) {
+                a0 += __double_as_longlong(my_delta[0]);
+                a1 = __dadd_rn(a1, my_delta[1]);
+                a2 = __dadd_rn(a2, my_delta[2]);
+            }
             __syncwarp();
         }
     }
@@ -311,6 +413,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         if (zeros) atomicAdd(&ctrl->zero_count, zeros);
         if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
     }
+    if (MOM) moments_finish(a0, a1, a2, ctrl, part0, part1, part2, m0, m1, m2);
 }
 
 }  // namespace sdmk

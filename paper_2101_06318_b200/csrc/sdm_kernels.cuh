@@ -367,8 +367,16 @@ __global__ void k_pairs_by_position(int64_t *__restrict__ xi, double *__restrict
 // ---------------------------------------------------------------------------------------------
 // Fused path (cell-contiguous storage): row a2 by boundary detection, rows a1,a3-a6 per cell
 // ---------------------------------------------------------------------------------------------
-__global__ void k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
-                                    int n_cell, int *__restrict__ cell_start)
+// cell_id is non-decreasing: cell c starts where the id first reaches c.  Every thread inspects four
+// consecutive droplets (one 16-byte load) and the one before them; writes happen only at boundaries.
+__device__ __forceinline__ void cell_boundary(int prev, int c, int i, int *__restrict__ cell_start)
+{
+    for (int cc = prev + 1; cc <= c; ++cc) cell_start[cc] = i;     // also fills empty cells
+}
+
+__global__ void __launch_bounds__(256)
+k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell,
+                    int *__restrict__ cell_start)
 {
     const int n = ctrl->n;
     if (n == 0) {
@@ -376,12 +384,31 @@ __global__ void k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl
             cell_start[c] = 0;
         return;
     }
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        int c = cell[i];
-        int prev = (i > 0) ? cell[i - 1] : -1;
-        for (int cc = prev + 1; cc <= c; ++cc) cell_start[cc] = i;
-        if (i == n - 1)
-            for (int cc = c + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
+    const int n4 = (n + 3) >> 2;
+    const int4 *cell4 = reinterpret_cast<const int4 *>(cell);
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += gridDim.x * blockDim.x) {
+        const int i = t << 2;
+        int c0, c1, c2, c3;
+        if (i + 3 < n) {
+            const int4 q = __ldcs(cell4 + t);
+            c0 = q.x; c1 = q.y; c2 = q.z; c3 = q.w;
+        } else {
+            c0 = cell[i];
+            c1 = (i + 1 < n) ? cell[i + 1] : c0;
+            c2 = (i + 2 < n) ? cell[i + 2] : c1;
+            c3 = c2;
+        }
+        const int prev = (i > 0) ? __ldg(cell + i - 1) : -1;
+        if (prev != c3) {                                           // some boundary among the four
+            if (c0 != prev) cell_boundary(prev, c0, i, cell_start);
+            if (c1 != c0) cell_boundary(c0, c1, i + 1, cell_start);
+            if (c2 != c1) cell_boundary(c1, c2, i + 2, cell_start);
+            if (c3 != c2) cell_boundary(c2, c3, i + 3, cell_start);
+        }
+        if (i + 4 >= n) {                                           // the thread holding the last droplet
+            const int last = (i + 3 < n) ? c3 : ((i + 2 < n) ? c2 : ((i + 1 < n) ? c1 : c0));
+            for (int cc = last + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
+        }
     }
 }
 
@@ -490,38 +517,31 @@ __global__ void k_compact_finalize(Ctrl *ctrl)
 // ---------------------------------------------------------------------------------------------
 // Row a8: moments M0 = sum xi (int64), M1 = sum xi v, M2 = sum xi v^2 (fp64)
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kMomentThreads)
-k_moments_global(const int64_t *__restrict__ xi, const double *__restrict__ v, Ctrl *ctrl,
-                 int64_t *__restrict__ part0, double *__restrict__ part1, double *__restrict__ part2,
-                 int64_t *__restrict__ m0, double *__restrict__ m1, double *__restrict__ m2)
+// CTA-level finish shared by the moment kernels: per-thread partial sums -> one partial per CTA ->
+// the last CTA to arrive sums all partials in a fixed order (run-to-run deterministic) and writes
+// the three results.  Every thread of the CTA must call it.
+__device__ __forceinline__ void moments_finish(int64_t a0, double a1, double a2, Ctrl *ctrl,
+                                               int64_t *__restrict__ part0, double *__restrict__ part1,
+                                               double *__restrict__ part2, int64_t *__restrict__ m0,
+                                               double *__restrict__ m1, double *__restrict__ m2)
 {
-    __shared__ int64_t s0[kMomentThreads / 32];
-    __shared__ double s1[kMomentThreads / 32], s2[kMomentThreads / 32];
+    constexpr int kMaxWarps = 32;
+    __shared__ int64_t s0[kMaxWarps];
+    __shared__ double s1[kMaxWarps], s2[kMaxWarps];
     __shared__ bool s_last;
-    const int n = ctrl->n;
-    int64_t a0 = 0;
-    double a1 = 0.0, a2 = 0.0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        int64_t x = xi[i];
-        double vol = v[i];
-        double xv = __dmul_rn(__ll2double_rn(x), vol);
-        a0 += x;
-        a1 = __dadd_rn(a1, xv);
-        a2 = __dadd_rn(a2, __dmul_rn(xv, vol));
-    }
+    const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = (blockDim.x + 31) >> 5;
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
         a0 += __shfl_down_sync(0xffffffffu, a0, d);
         a1 += __shfl_down_sync(0xffffffffu, a1, d);
         a2 += __shfl_down_sync(0xffffffffu, a2, d);
     }
-    const int lane = lane_id(), warp = threadIdx.x >> 5;
     if (lane == 0) { s0[warp] = a0; s1[warp] = a1; s2[warp] = a2; }
     __syncthreads();
     if (threadIdx.x == 0) {
         int64_t b0 = 0;
         double b1 = 0.0, b2 = 0.0;
-        for (int w = 0; w < kMomentThreads / 32; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
+        for (int w = 0; w < n_warps; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
         part0[blockIdx.x] = b0; part1[blockIdx.x] = b1; part2[blockIdx.x] = b2;
         __threadfence();
         unsigned int done = atomicAdd(&ctrl->moment_done, 1u);
@@ -529,7 +549,6 @@ k_moments_global(const int64_t *__restrict__ xi, const double *__restrict__ v, C
     }
     __syncthreads();
     if (!s_last) return;
-    // the last CTA sums the per-CTA partials in a fixed order: the result is run-to-run deterministic
     __threadfence();
     a0 = 0; a1 = 0.0; a2 = 0.0;
     for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) {
@@ -549,10 +568,41 @@ k_moments_global(const int64_t *__restrict__ xi, const double *__restrict__ v, C
     if (threadIdx.x == 0) {
         int64_t b0 = 0;
         double b1 = 0.0, b2 = 0.0;
-        for (int w = 0; w < kMomentThreads / 32; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
+        for (int w = 0; w < n_warps; ++w) { b0 += s0[w]; b1 += s1[w]; b2 += s2[w]; }
         *m0 = b0; *m1 = b1; *m2 = b2;
         ctrl->moment_done = 0;
     }
+}
+
+__global__ void __launch_bounds__(kMomentThreads)
+k_moments_global(const int64_t *__restrict__ xi, const double *__restrict__ v, Ctrl *ctrl,
+                 int64_t *__restrict__ part0, double *__restrict__ part1, double *__restrict__ part2,
+                 int64_t *__restrict__ m0, double *__restrict__ m1, double *__restrict__ m2)
+{
+    const int n = ctrl->n;
+    int64_t a0 = 0;
+    double a1 = 0.0, a2 = 0.0;
+    // two droplets per thread and iteration: 16-byte loads (both arrays are 256-byte aligned)
+    const int n2 = n >> 1;
+    const longlong2 *xi2 = reinterpret_cast<const longlong2 *>(xi);
+    const double2 *v2 = reinterpret_cast<const double2 *>(v);
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n2; t += gridDim.x * blockDim.x) {
+        const longlong2 x = __ldcs(xi2 + t);
+        const double2 vol = __ldcs(v2 + t);
+        const double xv0 = __dmul_rn(__ll2double_rn(x.x), vol.x), xv1 = __dmul_rn(__ll2double_rn(x.y), vol.y);
+        a0 += x.x + x.y;
+        a1 = __dadd_rn(a1, __dadd_rn(xv0, xv1));
+        a2 = __dadd_rn(a2, __dadd_rn(__dmul_rn(xv0, vol.x), __dmul_rn(xv1, vol.y)));
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t x = xi[n - 1];
+        const double vol = v[n - 1];
+        const double xv = __dmul_rn(__ll2double_rn(x), vol);
+        a0 += x;
+        a1 = __dadd_rn(a1, xv);
+        a2 = __dadd_rn(a2, __dmul_rn(xv, vol));
+    }
+    moments_finish(a0, a1, a2, ctrl, part0, part1, part2, m0, m1, m2);
 }
 
 __global__ void k_moments_zero(int n_cell, int64_t *__restrict__ m0, double *__restrict__ m1,

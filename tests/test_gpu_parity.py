@@ -34,13 +34,20 @@ def _make(sdm_mod, w, capacity=None, options=()):
     return s
 
 
-def _compare_step(s, xi, v, cell, w, step, check_perm=True):
+def _compare_step(s, xi, v, cell, w, step, check_perm=True, fused_moments=False):
     """Advance both sides by one [remove_zero; step] and compare everything."""
     xi, v, cell = oracle.remove_zero(xi, v, cell)
     n_gpu = s.remove_zero()
     assert n_gpu == len(xi), f"survivor count differs at step {step}"
     idx, cs, nev = oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
-    s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    if fused_moments:
+        m0, m1, m2 = (t.cpu().numpy()[0] for t in
+                      s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step))
+        o0, o1, o2 = oracle.moments(xi, v)
+        assert int(m0) == o0, f"M0 differs at step {step}"
+        assert abs(m1 - o1) <= 1e-12 * o1 and abs(m2 - o2) <= 1e-12 * o2, f"moments differ at step {step}"
+    else:
+        s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
     gxi, gv, gc = (t.cpu().numpy() for t in s.get_state())
     assert np.array_equal(gc, cell), f"cell ids differ at step {step}"
     if check_perm:
@@ -60,7 +67,8 @@ def _run_parity(sdm_mod, w, steps, options=(), expect_mode=None):
     xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
     events = 0
     for step in range(steps):
-        xi, v, cell, nev = _compare_step(s, xi, v, cell, w, step)
+        # every other step goes through the fused step+moments entry point
+        xi, v, cell, nev = _compare_step(s, xi, v, cell, w, step, fused_moments=(step % 2 == 1))
         events += nev
     cnt = s.counters()
     assert cnt["events"] == events and cnt["n_sd"] == len(xi)
@@ -158,6 +166,22 @@ def test_tiny_segment_cap_exercises_the_counting_fallback(sdm_mod):
     _run_parity(sdm_mod, w, 4, options=[(sdm_mod.OPT_SEGMENT_CAP, 8)], expect_mode=0)
     w = _ragged_workload([8, 3, 0, 7, 1, 8], seed=6, shuffled=False)
     _run_parity(sdm_mod, w, 4, options=[(sdm_mod.OPT_SEGMENT_CAP, 8)], expect_mode=1)
+
+
+def test_screening_off_gives_identical_results(sdm_mod):
+    w = workloads.grid_uniform(8, 8, 256, seed=4)
+    w.dV = 2.0
+    a = _make(sdm_mod, w)
+    b = _make(sdm_mod, w, options=[(sdm_mod.OPT_SCREENING, 0)])
+    for step in range(4):
+        a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 3, step)
+        b.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 3, step)
+    for ta, tb in zip(a.get_state(), b.get_state()):
+        assert torch.equal(ta, tb)
+    ca, cb = a.counters(), b.counters()
+    assert ca["events"] == cb["events"] > 0
+    assert ca["exact_evals"] < cb["exact_evals"] == 4 * 64 * 128     # screening skipped most evaluations
+    a.close(), b.close()
 
 
 def test_empty_and_single_droplet_states(sdm_mod):
@@ -289,3 +313,51 @@ def test_results_do_not_depend_on_step_order_of_calls_only_on_seed_and_step(sdm_
     a.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, 1, 18)
     assert not torch.equal(x1, a.get_state()[0])
     a.close()
+
+
+def test_c5_full_size_sampled_parity_in_bench_configuration(sdm_mod):
+    """BASELINE.json config 5 at full size (2^26 droplets), driven exactly like bench.py's timed
+    step; the oracle recomputes sampled cells one by one (cells are independent and the RNG counter
+    is the global storage index), and size-independent properties are checked on the whole state."""
+    w = workloads.grid_uniform(512, 512, 256, seed=0)
+    w.dV = 1e3 / 40.0                 # 40x denser than C5 so that the sampled cells see events in two steps
+    s = sdm_mod.SDM(w.n_sd, w.n_cell)
+    s.set_state_host(torch.from_numpy(w.xi).pin_memory(), torch.from_numpy(w.v).pin_memory(),
+                     torch.from_numpy(w.cell_id).pin_memory())
+    assert s.counters()["mode"] == 1
+    mom = s.moments()
+    n_steps = 2
+    for step in range(n_steps):
+        s.remove_zero(sync=False)
+        s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step, out=mom)
+    gidx, gcs = s.get_permutation(w.n_sd)
+    gxi, gv, gc = s.get_state()
+    n = gxi.shape[0]
+    assert n == w.n_sd                                     # xi = 1e6: nothing can reach zero in two steps
+    # whole-state properties
+    assert torch.equal(torch.sort(gidx.long()).values, torch.arange(n, device="cuda"))
+    assert torch.equal(gidx // 256, torch.arange(n, device="cuda", dtype=torch.int32) // 256)
+    assert torch.equal(gcs.long(), torch.arange(w.n_cell + 1, device="cuda") * 256)
+    hxi, hv = gxi.cpu().numpy(), gv.cpu().numpy()
+    assert int(mom[0].cpu()[0]) == int(hxi.sum())
+    m1_0 = oracle.moments(w.xi, w.v)[1]
+    assert abs(float(mom[1].cpu()[0]) - m1_0) <= 1e-12 * m1_0          # water is conserved
+    assert np.all(hv >= w.v) and np.all(hxi <= w.xi) and np.all(hxi > 0)
+    # sampled cells, recomputed by the oracle from the initial state
+    rng = np.random.default_rng(123)
+    changed_cells = np.unique(np.nonzero(hxi != w.xi)[0] // 256)
+    sample = np.concatenate([rng.integers(0, w.n_cell, 40), changed_cells[:24], [0, w.n_cell - 1]])
+    hidx = gidx.cpu().numpy()
+    events = 0
+    for c in sample:
+        lo, hi = int(c) * 256, int(c) * 256 + 256
+        xs, vs = w.xi[lo:hi].copy(), w.v[lo:hi].copy()
+        sid = np.arange(lo, hi, dtype=np.int64)
+        zc = np.zeros(256, dtype=np.int32)
+        for step in range(n_steps):
+            li, _, nev = oracle.step(xs, vs, zc, 1, w.dt, w.dV, w.kernel, w.kparam, w.seed, step, sid=sid)
+            events += nev
+        assert np.array_equal(lo + li, hidx[lo:hi]), f"permutation of cell {c}"
+        assert np.array_equal(xs, hxi[lo:hi]) and np.array_equal(vs, hv[lo:hi]), f"state of cell {c}"
+    assert events >= 24
+    s.close()
