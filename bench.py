@@ -181,6 +181,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lanes", type=int, default=0, help="tuning: lanes per cell of the fused kernel (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -209,6 +210,8 @@ def main():
     hc = torch.from_numpy(w.cell_id).pin_memory()
     s.set_state_host(hx, hv, hc)
     s.set_option(pkg.OPT_TIMING, 1)
+    if args.lanes:
+        s.set_option(pkg.OPT_LANES_PER_CELL, args.lanes)
     mode = s.counters()["mode"]
     mom = s.moments()
 

@@ -51,7 +51,8 @@ enum {
     SDM_OPT_SEGMENT_CAP = 2,   /* [0] >0: override the largest segment a warp sorts on chip (tests) */
     SDM_OPT_WRITE_IDX = 3,     /* [1] 0: do not export the permutation (idx is then undefined)      */
     SDM_OPT_SCREENING = 4,     /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
-    SDM_OPT_TIMING = 5         /* [0] 1: bracket the dominant kernel of each step with CUDA events   */
+    SDM_OPT_TIMING = 5,        /* [0] 1: bracket the dominant kernel of each step with CUDA events   */
+    SDM_OPT_LANES_PER_CELL = 6 /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)          */
 };
 
 /* Counter slots returned by sdm_get_counters. */

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     OPT_WRITE_IDX,
     OPT_SCREENING,
     OPT_TIMING,
+    OPT_LANES_PER_CELL,
     load_library,
     library_path,
     workspace_bytes,

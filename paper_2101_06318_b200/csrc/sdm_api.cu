@@ -94,6 +94,7 @@ struct sdm {
     int seg_cap = kWarpCap;
     bool write_idx = true;
     bool screening = true;
+    int lanes_per_cell = 0;      // 0: automatic
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
     size_t ev_used = 0;
@@ -210,22 +211,32 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     if (use_fused(h)) {
         SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 3) / 4, 256, 32), 256, 0, h->cell, h->ctrl, h->n_cell,
                    h->cell_start);
-        const int gf = grid_for(h, (int64_t)h->n_cell * 32, kFusedWarps * 32, 8);
-#define SDM_FUSED(EE)                                                                                    \
-    do {                                                                                                 \
-        if (m0)                                                                                          \
-            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, true>), gf, kFusedWarps * 32, 0, h->xi, h->v,   \
-                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,   \
-                                    h->part2, m0, m1, m2));                                              \
-        else                                                                                             \
-            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, false>), gf, kFusedWarps * 32, 0, h->xi, h->v,  \
-                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,   \
-                                    h->part2, m0, m1, m2));                                              \
+        // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
+        // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose
+        // more to instruction fetch than they save in shuffles (measured).
+        int E = 8, L = 8;
+        if (h->max_count > 256) { E = 16; L = 32; }
+        else if (h->max_count > 128) { E = 8; L = 32; }
+        else if (h->max_count > 64) { E = 8; L = 16; }
+        if (h->lanes_per_cell == 16 && h->max_count > 128 && h->max_count <= 256) { E = 16; L = 16; }
+        const int64_t warps_needed = ((int64_t)h->n_cell * L + 31) / 32;
+        const int gf = grid_for(h, warps_needed * 32, kFusedWarps * 32, 8);
+#define SDM_FUSED(EE, LL)                                                                                    \
+    do {                                                                                                     \
+        if (m0)                                                                                              \
+            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, true>), gf, kFusedWarps * 32, 0, h->xi, h->v,   \
+                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,       \
+                                    h->part2, m0, m1, m2));                                                  \
+        else                                                                                                 \
+            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, false>), gf, kFusedWarps * 32, 0, h->xi, h->v,  \
+                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,       \
+                                    h->part2, m0, m1, m2));                                                  \
     } while (0)
-        if (h->max_count <= 64) SDM_FUSED(2);
-        else if (h->max_count <= 128) SDM_FUSED(4);
-        else if (h->max_count <= 256) SDM_FUSED(8);
-        else SDM_FUSED(16);
+        if (E == 8 && L == 8) SDM_FUSED(8, 8);
+        else if (E == 8 && L == 16) SDM_FUSED(8, 16);
+        else if (E == 8 && L == 32) SDM_FUSED(8, 32);
+        else if (E == 16 && L == 16) SDM_FUSED(16, 16);
+        else SDM_FUSED(16, 32);
 #undef SDM_FUSED
         return SDM_OK;
     }
@@ -416,6 +427,10 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
     case SDM_OPT_WRITE_IDX: h->write_idx = value != 0; return SDM_OK;
     case SDM_OPT_SCREENING: h->screening = value != 0; return SDM_OK;
     case SDM_OPT_TIMING: h->timing = value != 0; h->ev_used = 0; return SDM_OK;
+    case SDM_OPT_LANES_PER_CELL:
+        if (value != 0 && value != 16) return fail(h, SDM_EINVAL, "lanes per cell: 0 or 16");
+        h->lanes_per_cell = (int)value;
+        return SDM_OK;
     default: return fail(h, SDM_EINVAL, "unknown option");
     }
 }

@@ -1,17 +1,24 @@
 // sdm_fused.cuh -- the dominant kernel: one SDM coalescence step on cell-contiguous storage.
 //
-// One warp owns one cell (E droplets per lane, cell capacity N = 32*E).  Per cell:
+// A group of L lanes owns one cell (E droplets per lane, cell capacity N = L*E; a warp works on
+// 32/L cells at once).  Per cell:
 //   1. stream xi, v once (coalesced, evict-first) and reduce an upper bound of the largest
 //      multiplicity and volume of the cell -> P_cell, an upper bound of Eq. 3 for EVERY pair the
-//      permutation could form in this cell ("screening", below);
+//      permutation could form in this cell ("screening", below); with MOM the same values feed the
+//      moment sums;
 //   2. one Philox4x32-10 block per droplet (row a1) -> a packed 32-bit sort word
-//      (top key bits | local index) and a flag "this droplet, as first-in-pair, could fire";
-//   3. register-resident bitonic network over the 32*E packed words: in-lane min/max for strides
+//      (top key bits | local index) and the smallest top uniform word of the lane;
+//   3. register-resident bitonic network over the N packed words: in-lane min/max for strides
 //      < E, __shfl_xor for lane strides (row a3); words that tie on the truncated key are put in
-//      exact (key64, storage index) order by a rare warp-uniform slow path, so idx is bit-exact;
+//      exact (key64, storage index) order by a rare slow path, so idx is bit-exact;
 //   4. idx written as vectors (row a3 output); pairs (2m, 2m+1) sit in one lane (row a4);
 //   5. only pairs whose first member is flagged evaluate Eq. 3-6 in fp64 (rows a5-a6), exactly as
 //      collide_pair_exact does for every pair on the general path.
+//
+// Why this shape: the kernel is bound by the integer ALU pipe (min/max of the sorting network, the
+// xors of Philox), not by HBM.  A compare-exchange between lanes costs a shuffle and two ALU
+// instructions per word, one inside a lane costs one, so cells are given to as few lanes as the
+// register file allows.
 //
 // Screening keeps results bit-identical: gamma = floor(p) + [u < p - floor(p)] is 0 whenever
 // p < 1 and u >= p.  P_cell >= p holds for every pair of the cell because K is bounded through the
@@ -25,22 +32,18 @@
 
 namespace sdmk {
 
-#ifndef SDM_FUSED_WARPS
-#define SDM_FUSED_WARPS 8
-#endif
-#ifndef SDM_FUSED_MIN_BLOCKS
-#define SDM_FUSED_MIN_BLOCKS 3
-#endif
-constexpr int kFusedWarps = SDM_FUSED_WARPS;
-constexpr int kFusedMinBlocks = SDM_FUSED_MIN_BLOCKS;
+constexpr int kFusedWarps = 8;
 
-template <int E>
-__device__ __forceinline__ void warp_sort_packed(uint32_t (&x)[E], int lane)
+// Bitonic network over N = L*E words held as x[r] at position (lane_in_group*E + r); every
+// compare-exchange puts the minimum at the lower position.  Masks stay below L, so shuffles never
+// leave the group.
+template <int E, int L>
+__device__ __forceinline__ void group_sort_packed(uint32_t (&x)[E], int lane)
 {
-    constexpr int N = 32 * E;
+    constexpr int N = L * E;
 #pragma unroll
     for (int k = 2; k <= N; k <<= 1) {
-        // first stage of the merge: partner p ^ (k-1), minimum to the lower position
+        // first stage of the merge: partner p ^ (k-1)
         if (k <= E) {
 #pragma unroll
             for (int r = 0; r < E; ++r) {
@@ -109,47 +112,41 @@ __device__ __forceinline__ uint32_t flag_threshold(double P)
 }
 
 // Rare: some adjacent sorted words tie on the truncated key.  Re-rank every tie run by the exact
-// (key64, local index) order.  sk: the N sorted words in warp-private shared memory (in/out).
-// Works on shared memory only, so that the caller's register arrays never get their address taken.
-__device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int s, int n_s, int lane, uint64_t seed,
+// (key64, local index) order.  sk: this group's N sorted words in shared memory (in/out).
+// Works on shared memory only, so that the caller's register arrays never
+// get their address taken.  Called by the whole warp (every group with its own cell).
+__device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int N, int s, int n_s, int li, uint64_t seed,
                                           uint64_t step)
 {
-    const uint32_t N = 32u * (uint32_t)E;
     PhiloxKey rk;
     philox_round_keys(seed, rk);
-    // pass 1: new position of each of this lane's words (kept in the upper half of the scratch)
-    uint32_t *np = sk + N;
+    uint32_t mine[32], dst[32];
     for (int r = 0; r < E; ++r) {
-        const int p = lane * E + r;
-        np[p] = (uint32_t)p;
-        if (p >= n_s) continue;
+        const int p = li * E + r;
         const uint32_t me = sk[p];
+        mine[r] = me;
+        dst[r] = (uint32_t)p;
+        if (p >= n_s) continue;
         int a = p, b = p + 1;
-        while (a > 0 && ((sk[a - 1] ^ me) < N)) --a;
-        while (b < n_s && ((sk[b] ^ me) < N)) ++b;
+        while (a > 0 && ((sk[a - 1] ^ me) < (uint32_t)N)) --a;
+        while (b < n_s && ((sk[b] ^ me) < (uint32_t)N)) ++b;
         if (b - a < 2) continue;
-        const int l = (int)(me & (N - 1));
+        const int l = (int)(me & (uint32_t)(N - 1));
         const uint64_t key = block_key64(droplet_block((uint32_t)(s + l), step, rk));
         int rank = 0;
         for (int q = a; q < b; ++q) {
             if (q == p) continue;
-            const int l2 = (int)(sk[q] & (N - 1));
+            const int l2 = (int)(sk[q] & (uint32_t)(N - 1));
             const uint64_t key2 = block_key64(droplet_block((uint32_t)(s + l2), step, rk));
             rank += key_less(key2, l2, key, l) ? 1 : 0;
         }
-        np[p] = (uint32_t)(a + rank);
+        dst[r] = (uint32_t)(a + rank);
     }
-    __syncwarp();
-    // pass 2: permute (read everything first, then write)
-    uint32_t mine[16], dst[16];
-    for (int r = 0; r < E; ++r) { mine[r] = sk[lane * E + r]; dst[r] = np[lane * E + r]; }
-    __syncwarp();
+    __syncwarp();                                     // everybody has read; now permute in place
     for (int r = 0; r < E; ++r) sk[dst[r]] = mine[r];
     __syncwarp();
 }
 
-// Rare: the cell has flagged droplets.  Evaluate rows a5-a6 exactly for the pairs they lead.
-// sk: sorted words, sflag: one ballot word per element slot k (bit = lane), both in shared memory.
 // One pair's contribution to (M0, M1, M2), products rounded as in k_moments_global.
 __device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v, int a, int b, int64_t &p0,
                                              double &p1, double &p2)
@@ -162,25 +159,28 @@ __device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v,
     p2 = __dadd_rn(__dmul_rn(ya, va), __dmul_rn(yb, vb));
 }
 
-// delta (may be NULL): three doubles of warp-private shared memory per lane; receives the change of
-// (M0, M1, M2) caused by this lane's events (M0 as a double holding an exact integer < 2^53 is not
-// enough in general, so M0's change is stored as the bit pattern of an int64).
-__device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int64_t *xi,
-                                            double *v, int s, int n_s, int lane, double dtdv, int32_t ktype,
-                                            double kparam, uint64_t seed, uint64_t step, double *delta)
+// Rare: the cell has flagged droplets.  Evaluate rows a5-a6 exactly for the pairs they lead.
+// sk: the group's sorted words; sflag[k]: ballot word of element slot k (bit = lane of the warp);
+// lane0: first lane of the group.  delta (may be NULL): three doubles per lane receiving the change
+// of (M0, M1, M2) caused by this lane's events (M0's change as the bit pattern of an int64).
+__device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int L, int lane0,
+                                            int64_t *xi, double *v, int s, int n_s, int li, double dtdv,
+                                            int32_t ktype, double kparam, uint64_t seed, uint64_t step,
+                                            double *delta)
 {
+    const uint32_t N = (uint32_t)(E * L);
     int64_t d0 = 0;
     double d1 = 0.0, d2 = 0.0;
-    const uint32_t N = 32u * (uint32_t)E;
     PhiloxKey rk;
     philox_round_keys(seed, rk);
     const double norm = pair_norm(n_s, dtdv);
     int packed = 0;                                   // events | zeros << 10 | exact << 20
     for (int m = 0; m < E / 2; ++m) {
-        const int p = lane * E + 2 * m;
+        const int p = li * E + 2 * m;
         if (p + 1 >= n_s) continue;
         const int a = (int)(sk[p] & (N - 1)), b = (int)(sk[p + 1] & (N - 1));
-        if (((sflag[a >> 5] >> (a & 31)) & 1u) == 0) continue;
+        // droplet a was element slot a / L of lane lane0 + a % L
+        if (((sflag[a / L] >> (lane0 + a % L)) & 1u) == 0) continue;
         const double u = block_uniform(droplet_block((uint32_t)(s + a), step, rk));
         int64_t o0 = 0;
         double o1 = 0.0, o2 = 0.0;
@@ -205,7 +205,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 }
 
 // Cells larger than the kernel's capacity cannot reach it (the host checks the largest cell at
-// sdm_set_state and cells never grow); this keeps the result defined anyway.
+// sdm_set_state and cells never grow); this keeps the result defined anyway.  Whole warp, one cell.
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
                                           double dtdv, int32_t ktype, double kparam, uint64_t seed,
                                           uint64_t step, double *delta)
@@ -241,83 +241,84 @@ __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int 
     return packed;
 }
 
+template <int E>
+struct FusedTraits {
+        static constexpr int kMinBlocks = (E >= 16) ? 2 : 3;
+};
+
 // MOM: also produce the global moments (M0, M1, M2) of the state AFTER the step: the pre-step sums
 // are taken from the values streamed for the screening, and every event adds its exact change.
-template <int E, bool MOM>
-__global__ void __launch_bounds__(kFusedWarps * 32, kFusedMinBlocks)
+template <int E, int L, bool MOM>
+__global__ void __launch_bounds__(kFusedWarps * 32, FusedTraits<E>::kMinBlocks)
 k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
               int n_cell, int *__restrict__ idx, Ctrl *ctrl, StepParams prm, int64_t *__restrict__ part0,
               double *__restrict__ part1, double *__restrict__ part2, int64_t *__restrict__ m0,
               double *__restrict__ m1, double *__restrict__ m2)
 {
-    constexpr int N = 32 * E;
-    static_assert(E >= 2 && (E & (E - 1)) == 0, "E must be an even power of two");
-    __shared__ uint32_t s_scratch[kFusedWarps][2 * N];      // rare paths only
+    constexpr int N = L * E;                  // cell capacity
+    constexpr int G = 32 / L;                 // cells per warp
+    static_assert(E >= 2 && (E & (E - 1)) == 0 && (L & (L - 1)) == 0 && L <= 32, "bad shape");
+    __shared__ uint32_t s_scratch[kFusedWarps][G][N];         // rare paths only
     __shared__ uint32_t s_flags[kFusedWarps][E];
     __shared__ double s_delta[MOM ? kFusedWarps * 32 * 3 : 1];
     double *my_delta = MOM ? &s_delta[(threadIdx.x >> 5) * 96 + (threadIdx.x & 31) * 3] : nullptr;
     int64_t a0 = 0;
     double a1 = 0.0, a2 = 0.0;
     const int warp = threadIdx.x >> 5, lane = lane_id();
+    const int g = lane / L, li = lane % L, lane0 = g * L;
     PhiloxKey rk;
     philox_round_keys(prm.seed, rk);
     int events = 0, zeros = 0, exact = 0;
-    const int warps_total = gridDim.x * kFusedWarps;
-    for (int c = blockIdx.x * kFusedWarps + warp; c < n_cell; c += warps_total) {
-        const int s = cell_start[c];
-        const int n_s = cell_start[c + 1] - s;
-        if (n_s <= 1) {
-            if (n_s == 1 && lane == 0) {
-                if (prm.write_idx) idx[s] = s;
-                if (MOM) {
-                    const int64_t x1 = xi[s];
-                    const double v1 = v[s], xv = __dmul_rn(__ll2double_rn(x1), v1);
-                    a0 += x1;
-                    a1 = __dadd_rn(a1, xv);
-                    a2 = __dadd_rn(a2, __dmul_rn(xv, v1));
-                }
-            }
-            continue;
+    const int cells_per_round = gridDim.x * kFusedWarps * G;
+    for (int cbase = (blockIdx.x * kFusedWarps + warp) * G; cbase < n_cell; cbase += cells_per_round) {
+        const int c = cbase + g;
+        int s = 0, n_s = 0;
+        if (c < n_cell) {
+            s = cell_start[c];
+            n_s = cell_start[c + 1] - s;
         }
-        if (n_s > N) {
-            const int pk = oversize_cell(xi, v, idx, s, n_s, lane, prm.dtdv, prm.kernel, prm.kparam, prm.seed,
-                                         prm.step, my_delta);
-            events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
-            if (MOM) {
-                a0 += __double_as_longlong(my_delta[0]);
-                a1 = __dadd_rn(a1, my_delta[1]);
-                a2 = __dadd_rn(a2, my_delta[2]);
+        if (__any_sync(0xffffffffu, n_s > N)) {
+            for (int gg = 0; gg < G; ++gg) {
+                const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
+                if (n2 <= N) continue;
+                const int pk = oversize_cell(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
+                                             prm.seed, prm.step, my_delta);
+                events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
+                if (MOM) {
+                    a0 += __double_as_longlong(my_delta[0]);
+                    a1 = __dadd_rn(a1, my_delta[1]);
+                    a2 = __dadd_rn(a2, my_delta[2]);
+                }
+                __syncwarp();
             }
-            continue;
+            if (n_s > N) n_s = 0;                 // done
         }
         // 1. stream the cell once: bounds of max xi and max v (volumes are positive doubles, so the
-        //    high word orders them; multiplicities are rounded up to fp32)
+        //    high word orders them; multiplicities are rounded up to fp32); moment sums with MOM
         uint32_t vhi_max = 0;
         float xi_max = 0.0f;
-        const int nrem = n_s - lane;                      // droplet k*32+lane exists iff nrem > 32k
+        const int nrem = n_s - li;                        // droplet k*L+li exists iff nrem > k*L
         if (prm.screening || MOM) {
-            int64_t lx[E];
-            double lv[E];
-            const long long *px = reinterpret_cast<const long long *>(xi + s + lane);
-            const double *pv = v + s + lane;
+            const long long *px = reinterpret_cast<const long long *>(xi + s + li);
+            const double *pv = v + s + li;
 #pragma unroll
             for (int k = 0; k < E; ++k) {
-                lx[k] = (nrem > 32 * k) ? __ldcs(px + 32 * k) : 0;
-                lv[k] = (nrem > 32 * k) ? __ldcs(pv + 32 * k) : 0.0;
-            }
-#pragma unroll
-            for (int k = 0; k < E; ++k) {
-                vhi_max = max(vhi_max, (uint32_t)__double2hiint(lv[k]));
-                xi_max = fmaxf(xi_max, __ll2float_ru(lx[k]));
+                const int64_t lx = (nrem > L * k) ? __ldcs(px + L * k) : 0;
+                const double lv = (nrem > L * k) ? __ldcs(pv + L * k) : 0.0;
+                vhi_max = max(vhi_max, (uint32_t)__double2hiint(lv));
+                xi_max = fmaxf(xi_max, __ll2float_ru(lx));
                 if (MOM) {                                  // absent droplets were loaded as (0, 0.0)
-                    const double xv = __dmul_rn(__ll2double_rn(lx[k]), lv[k]);
-                    a0 += lx[k];
+                    const double xv = __dmul_rn(__ll2double_rn(lx), lv);
+                    a0 += lx;
                     a1 = __dadd_rn(a1, xv);
-                    a2 = __dadd_rn(a2, __dmul_rn(xv, lv[k]));
+                    a2 = __dadd_rn(a2, __dmul_rn(xv, lv));
                 }
             }
-            vhi_max = __reduce_max_sync(0xffffffffu, vhi_max);
-            xi_max = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(xi_max)));
+#pragma unroll
+            for (int d = 1; d < L; d <<= 1) {
+                vhi_max = max(vhi_max, __shfl_xor_sync(0xffffffffu, vhi_max, d));
+                xi_max = fmaxf(xi_max, __shfl_xor_sync(0xffffffffu, xi_max, d));
+            }
         }
         uint32_t thr = 0xFFFFFFFFu;
         if (prm.screening) {
@@ -326,40 +327,40 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
                                                     pair_norm(n_s, prm.dtdv));
             thr = flag_threshold(P);
         }
-        // 2. Philox block per droplet -> packed sort word + flag
+        // 2. Philox block per droplet -> packed sort word; smallest top uniform word of the lane
         uint32_t x[E];
-        uint32_t umin = 0xFFFFFFFFu;                      // smallest top uniform word of this lane's droplets
-        const uint32_t sid0 = (uint32_t)(s + lane);
+        uint32_t umin = 0xFFFFFFFFu;
+        const uint32_t sid0 = (uint32_t)(s + li);
 #pragma unroll
         for (int k = 0; k < E; ++k) {
-            const uint4 w = droplet_block(sid0 + 32u * k, prm.step, rk);
-            const bool valid = nrem > 32 * k;
-            x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)(lane + 32 * k)) : 0xFFFFFFFFu;
+            const uint4 w = droplet_block(sid0 + (uint32_t)(L * k), prm.step, rk);
+            const bool valid = nrem > L * k;
+            x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)(li + L * k)) : 0xFFFFFFFFu;
             umin = min(umin, valid ? w.w : 0xFFFFFFFFu);
         }
         // 3. sort, then exact order inside truncated-key ties (rare)
-        warp_sort_packed<E>(x, lane);
+        group_sort_packed<E, L>(x, lane);
         {
             // words that share the truncated key differ by less than N (necessary, not sufficient:
             // the slow path re-checks); sorted ascending, so differences are non-negative
             const uint32_t nx = __shfl_down_sync(0xffffffffu, x[0], 1);
-            uint32_t dmin = (lane < 31) ? nx - x[E - 1] : 0xFFFFFFFFu;
+            uint32_t dmin = (li < L - 1) ? nx - x[E - 1] : 0xFFFFFFFFu;
 #pragma unroll
             for (int r = 0; r + 1 < E; ++r) dmin = min(dmin, x[r + 1] - x[r]);
             if (__any_sync(0xffffffffu, dmin < (uint32_t)N)) {
-                uint32_t *sk = s_scratch[warp];
+                uint32_t *sk = s_scratch[warp][g];
 #pragma unroll
-                for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
+                for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
                 __syncwarp();
-                fix_key_ties(sk, E, s, n_s, lane, prm.seed, prm.step);
+                fix_key_ties(sk, E, N, s, n_s, li, prm.seed, prm.step);
 #pragma unroll
-                for (int r = 0; r < E; ++r) x[r] = sk[lane * E + r];
+                for (int r = 0; r < E; ++r) x[r] = sk[li * E + r];
                 __syncwarp();
             }
         }
         // 4. idx
         if (prm.write_idx) {
-            const int p0 = lane * E;
+            const int p0 = li * E;
             if (((s & (N - 1)) == 0) && (E % 4 == 0) && (p0 + E <= n_s)) {
                 // cell start aligned to the capacity: s + local == s | local
 #pragma unroll
@@ -383,19 +384,19 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         }
         // 5. pairs led by a flagged droplet (rare)
         if (__any_sync(0xffffffffu, umin <= thr)) {
-            // rare: redo the blocks of this lane's droplets to learn which ones are flagged
+            // redo the blocks of this lane's droplets to learn which ones are flagged
 #pragma unroll 1
             for (int k = 0; k < E; ++k) {
-                const uint4 w = droplet_block(sid0 + 32u * k, prm.step, rk);
-                const uint32_t word = __ballot_sync(0xffffffffu, (nrem > 32 * k) && (w.w <= thr));
-                if (lane == k) s_flags[warp][k] = word;
+                const uint4 w = droplet_block(sid0 + (uint32_t)(L * k), prm.step, rk);
+                const uint32_t word = __ballot_sync(0xffffffffu, (nrem > L * k) && (w.w <= thr));
+                if (lane == (k & 31)) s_flags[warp][k] = word;
             }
-            uint32_t *sk = s_scratch[warp];
+            uint32_t *sk = s_scratch[warp][g];
 #pragma unroll
-            for (int r = 0; r < E; ++r) sk[lane * E + r] = x[r];
+            for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
             __syncwarp();
-            const int pk = collide_flagged(sk, s_flags[warp], E, xi, v, s, n_s, lane, prm.dtdv, prm.kernel,
-                                           prm.kparam, prm.seed, prm.step, my_delta);
+            const int pk = collide_flagged(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
+                                           prm.kernel, prm.kparam, prm.seed, prm.step, my_delta);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
             if (MOM) {
                 a0 += __double_as_longlong(my_delta[0]);

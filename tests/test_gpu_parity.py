@@ -361,3 +361,16 @@ def test_c5_full_size_sampled_parity_in_bench_configuration(sdm_mod):
         assert np.array_equal(xs, hxi[lo:hi]) and np.array_equal(vs, hv[lo:hi]), f"state of cell {c}"
     assert events >= 24
     s.close()
+
+
+@pytest.mark.parametrize("max_count,lanes", [(60, 0), (100, 0), (256, 0), (256, 16), (400, 0)])
+def test_every_shape_of_the_fused_kernel(sdm_mod, max_count, lanes):
+    """The per-cell kernel is instantiated for several (droplets per lane, lanes per cell) shapes,
+    chosen by the largest cell; each must give the oracle's result on ragged cells."""
+    rng = np.random.default_rng(max_count + lanes)
+    counts = rng.integers(0, max_count + 1, 37)
+    counts[5], counts[11], counts[20] = max_count, 1, 0
+    w = _ragged_workload(counts, seed=max_count, shuffled=False, kparam=0.3 / max_count)
+    opts = [(sdm_mod.OPT_LANES_PER_CELL, lanes)] if lanes else []
+    events, _ = _run_parity(sdm_mod, w, 5, options=opts, expect_mode=1)
+    assert events > 50
