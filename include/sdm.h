@@ -52,7 +52,10 @@ enum {
     SDM_OPT_WRITE_IDX = 3,     /* [1] 0: do not export the permutation (idx is then undefined)      */
     SDM_OPT_SCREENING = 4,     /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
     SDM_OPT_TIMING = 5,        /* [0] 1: bracket the dominant kernel of each step with CUDA events   */
-    SDM_OPT_LANES_PER_CELL = 6 /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)          */
+    SDM_OPT_LANES_PER_CELL = 6, /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)         */
+    SDM_OPT_SORT_ENGINE = 7,   /* [0] fused path, per-cell permutation: 0 automatic, 1 register sorting  */
+                               /*     network, 2 bucket sort on the top key bits (cells <= 256 only)     */
+    SDM_OPT_SORT_FALLBACK = 8  /* [0] 1: bucket sort always takes its histogram-overflow fallback (tests) */
 };
 
 /* Counter slots returned by sdm_get_counters. */

@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     OPT_SCREENING,
     OPT_TIMING,
     OPT_LANES_PER_CELL,
+    OPT_SORT_ENGINE,
+    OPT_SORT_FALLBACK,
     load_library,
     library_path,
     workspace_bytes,

@@ -15,8 +15,8 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libsdm.so")
 SOURCES = [os.path.join(CSRC, "sdm_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "sdm_kernels.cuh"), os.path.join(CSRC, "sdm_device.cuh"),
-                  os.path.join(ROOT, "include", "sdm.h")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cuh")] + [
+    os.path.join(ROOT, "include", "sdm.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -15,6 +15,7 @@
 
 #include "sdm_kernels.cuh"
 #include "sdm_fused.cuh"
+#include "sdm_fused_bucket.cuh"
 
 using namespace sdmk;
 
@@ -95,6 +96,8 @@ struct sdm {
     bool write_idx = true;
     bool screening = true;
     int lanes_per_cell = 0;      // 0: automatic
+    int sort_engine = 0;         // 0: automatic, 1: register sorting network, 2: bucket sort
+    bool sort_fallback = false;
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
     size_t ev_used = 0;
@@ -196,7 +199,7 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.seed = seed;
     prm.step = step;
     prm.screening = h->screening ? 1 : 0;
-    prm.scr_c = 0.0f;
+    prm.sort_fallback = h->sort_fallback ? 1 : 0;
     return SDM_OK;
 }
 
@@ -214,6 +217,20 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
         // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose
         // more to instruction fetch than they save in shuffles (measured).
+        const bool bucket = h->max_count <= kBucketCap &&
+                            (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
+        if (bucket) {
+            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kBucketWarps * 32, 3);
+            if (m0)
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_bucket<true>), gb, kBucketWarps * 32, 0, h->xi, h->v,
+                                        h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
+                                        h->part2, m0, m1, m2));
+            else
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_bucket<false>), gb, kBucketWarps * 32, 0, h->xi, h->v,
+                                        h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
+                                        h->part2, m0, m1, m2));
+            return SDM_OK;
+        }
         int E = 8, L = 8;
         if (h->max_count > 256) { E = 16; L = 32; }
         else if (h->max_count > 128) { E = 8; L = 32; }
@@ -431,6 +448,11 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         if (value != 0 && value != 16) return fail(h, SDM_EINVAL, "lanes per cell: 0 or 16");
         h->lanes_per_cell = (int)value;
         return SDM_OK;
+    case SDM_OPT_SORT_ENGINE:
+        if (value < 0 || value > 2) return fail(h, SDM_EINVAL, "sort engine: 0 (auto), 1 (network) or 2 (bucket)");
+        h->sort_engine = (int)value;
+        return SDM_OK;
+    case SDM_OPT_SORT_FALLBACK: h->sort_fallback = value != 0; return SDM_OK;
     default: return fail(h, SDM_EINVAL, "unknown option");
     }
 }

@@ -35,11 +35,11 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        uint32_t n0 = hi1 ^ c1 ^ rk.k0[r];
-        uint32_t n2 = hi0 ^ c3 ^ rk.k1[r];
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        // one 32x32->64 multiply per product (IMAD.WIDE.U32) instead of separate hi and lo halves
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[r];
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k1[r];
+        c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
     }
     return make_uint4(c0, c1, c2, c3);
 }
@@ -71,9 +71,8 @@ struct StepParams {
     int32_t kernel;   // SDM_KERNEL_*
     int32_t write_idx;
     uint64_t seed, step;
-    // fp32 screening (see pair_screen): upper bounds, 0 => screening disabled
-    float scr_c;      // upper bound of kparam(*pi)*dt/dV with margin
-    int32_t screening;
+    int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
+    int32_t sort_fallback;  // 1: force the counting fallback of the bucket sort (tests)
 };
 
 // R10: cube root as a fixed sequence of IEEE double operations (no division, no FMA).

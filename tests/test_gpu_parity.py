@@ -374,3 +374,18 @@ def test_every_shape_of_the_fused_kernel(sdm_mod, max_count, lanes):
     opts = [(sdm_mod.OPT_LANES_PER_CELL, lanes)] if lanes else []
     events, _ = _run_parity(sdm_mod, w, 5, options=opts, expect_mode=1)
     assert events > 50
+
+
+@pytest.mark.parametrize("max_count,engine,fallback", [(256, 2, 0), (256, 1, 0), (200, 2, 0), (100, 2, 0),
+                                                       (31, 2, 0), (256, 2, 1), (77, 2, 1)])
+def test_sort_engines_of_the_fused_kernel(sdm_mod, max_count, engine, fallback):
+    """Per-cell permutation by bucket sort on the top key bits (engine 2) or by the register sorting
+    network (engine 1): both must reproduce the oracle's argsort by (key64, storage index); the
+    bucket sort's histogram-overflow fallback is forced through SDM_OPT_SORT_FALLBACK."""
+    rng = np.random.default_rng(1000 + max_count + engine)
+    counts = rng.integers(0, max_count + 1, 53)
+    counts[3], counts[7], counts[19], counts[52] = max_count, 1, 0, max_count
+    w = _ragged_workload(counts, seed=max_count + engine, shuffled=False, kparam=0.3 / max_count)
+    opts = [(sdm_mod.OPT_SORT_ENGINE, engine), (sdm_mod.OPT_SORT_FALLBACK, fallback)]
+    events, _ = _run_parity(sdm_mod, w, 5, options=opts, expect_mode=1)
+    assert events > 50
