@@ -182,6 +182,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, help="tuning: lanes per cell of the fused kernel (0 = auto)")
+    ap.add_argument("--engine", type=int, default=0, help="tuning: per-cell sort engine (0 auto, 1 network, 2 bucket)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -212,6 +213,8 @@ def main():
     s.set_option(pkg.OPT_TIMING, 1)
     if args.lanes:
         s.set_option(pkg.OPT_LANES_PER_CELL, args.lanes)
+    if args.engine:
+        s.set_option(pkg.OPT_SORT_ENGINE, args.engine)
     mode = s.counters()["mode"]
     mom = s.moments()
 

@@ -15,7 +15,7 @@
 
 #include "sdm_kernels.cuh"
 #include "sdm_fused.cuh"
-#include "sdm_fused_bucket.cuh"
+#include "sdm_fused_count.cuh"
 
 using namespace sdmk;
 
@@ -217,16 +217,16 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
         // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose
         // more to instruction fetch than they save in shuffles (measured).
-        const bool bucket = h->max_count <= kBucketCap &&
+        const bool bucket = h->max_count <= kCountCap &&
                             (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
         if (bucket) {
-            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kBucketWarps * 32, 3);
+            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32, kCountBlocksPerSM);
             if (m0)
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_bucket<true>), gb, kBucketWarps * 32, 0, h->xi, h->v,
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, 0, h->xi, h->v,
                                         h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
                                         h->part2, m0, m1, m2));
             else
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_bucket<false>), gb, kBucketWarps * 32, 0, h->xi, h->v,
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<false>), gb, kCountWarps * 32, 0, h->xi, h->v,
                                         h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
                                         h->part2, m0, m1, m2));
             return SDM_OK;
