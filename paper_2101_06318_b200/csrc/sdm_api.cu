@@ -200,6 +200,7 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.step = step;
     prm.screening = h->screening ? 1 : 0;
     prm.sort_fallback = h->sort_fallback ? 1 : 0;
+    philox_round_keys(seed, prm.rk);
     return SDM_OK;
 }
 
@@ -222,11 +223,11 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         if (bucket) {
             const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32, kCountBlocksPerSM);
             if (m0)
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, 0, h->xi, h->v,
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
                                         h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
                                         h->part2, m0, m1, m2));
             else
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<false>), gb, kCountWarps * 32, 0, h->xi, h->v,
+                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<false>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
                                         h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
                                         h->part2, m0, m1, m2));
             return SDM_OK;
@@ -409,6 +410,10 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
     e = cudaFuncSetAttribute(k_segment_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort)");
+    e = cudaFuncSetAttribute(k_fused_cells_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<true>)");
+    e = cudaFuncSetAttribute(k_fused_cells_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<false>)");
     e = cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(ctrl)");
     e = cudaMemsetAsync(h->cell_start, 0, ((size_t)n_cell + 1) * 4, h->stream);

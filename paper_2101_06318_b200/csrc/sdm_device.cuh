@@ -18,7 +18,7 @@ struct PhiloxKey {          // the ten round keys, precomputed once per thread (
     uint32_t k0[10], k1[10];
 };
 
-__device__ __forceinline__ void philox_round_keys(uint64_t seed, PhiloxKey &rk)
+__host__ __device__ __forceinline__ void philox_round_keys(uint64_t seed, PhiloxKey &rk)
 {
     uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
 #pragma unroll
@@ -72,7 +72,9 @@ struct StepParams {
     int32_t write_idx;
     uint64_t seed, step;
     int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
-    int32_t sort_fallback;  // 1: force the counting fallback of the bucket sort (tests)
+    int32_t sort_fallback;  // unused (kept for ABI stability of the option numbering)
+    PhiloxKey rk;           // round keys of `seed`: kernels that take the parameters as __grid_constant__ read
+                            // them straight from the constant bank instead of holding 20 registers
 };
 
 // R10: cube root as a fixed sequence of IEEE double operations (no division, no FMA).
