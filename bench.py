@@ -182,6 +182,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, help="tuning: lanes per cell of the fused kernel (0 = auto)")
+    ap.add_argument("--ctas-per-sm", type=int, default=0, help="tuning: grid of the counting-sort kernel (0 = auto)")
     ap.add_argument("--engine", type=int, default=0, help="tuning: per-cell sort engine (0 auto, 1 network, 2 bucket)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -215,6 +216,8 @@ def main():
         s.set_option(pkg.OPT_LANES_PER_CELL, args.lanes)
     if args.engine:
         s.set_option(pkg.OPT_SORT_ENGINE, args.engine)
+    if args.ctas_per_sm:
+        s.set_option(pkg.OPT_CTAS_PER_SM, args.ctas_per_sm)
     mode = s.counters()["mode"]
     mom = s.moments()
 

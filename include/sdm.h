@@ -55,7 +55,8 @@ enum {
     SDM_OPT_LANES_PER_CELL = 6, /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)         */
     SDM_OPT_SORT_ENGINE = 7,   /* [0] fused path, per-cell permutation: 0 automatic, 1 register sorting  */
                                /*     network, 2 bucket sort on the top key bits (cells <= 256 only)     */
-    SDM_OPT_SORT_FALLBACK = 8  /* [0] 1: bucket sort always takes its histogram-overflow fallback (tests) */
+    SDM_OPT_SORT_FALLBACK = 8, /* [0] reserved (no effect)                                                */
+    SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count (scaling runs) */
 };
 
 /* Counter slots returned by sdm_get_counters. */

@@ -20,6 +20,7 @@ OPT_TIMING = 5
 OPT_LANES_PER_CELL = 6
 OPT_SORT_ENGINE = 7
 OPT_SORT_FALLBACK = 8
+OPT_CTAS_PER_SM = 9
 CNT_NAMES = ("n_sd", "events", "zeros", "launches", "mode", "max_cell", "exact_evals", "reserved")
 
 SDM_OK, SDM_EINVAL, SDM_ECAPACITY, SDM_ECUDA, SDM_ESTATE = 0, -1, -2, -3, -4

@@ -98,6 +98,7 @@ struct sdm {
     int lanes_per_cell = 0;      // 0: automatic
     int sort_engine = 0;         // 0: automatic, 1: register sorting network, 2: bucket sort
     bool sort_fallback = false;
+    int ctas_per_sm = 0;         // 0: the kernel's own choice (tuning / scaling experiments)
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
     size_t ev_used = 0;
@@ -221,7 +222,8 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         const bool bucket = h->max_count <= kCountCap &&
                             (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
         if (bucket) {
-            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32, kCountBlocksPerSM);
+            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32,
+                                    h->ctas_per_sm > 0 ? h->ctas_per_sm : kCountBlocksPerSM);
             if (m0)
                 SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
                                         h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
@@ -292,11 +294,9 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
 
 int enqueue_remove_zero(sdm_t *h)
 {
-    SDM_CUDA(h, cudaMemsetAsync(h->tile_status, 0, (size_t)h->L.n_tiles * 8, h->stream));
     int64_t tiles = (h->n_ub + kCompactTile - 1) / kCompactTile;
     SDM_LAUNCH(h, k_compact, grid_for(h, tiles * kCompactThreads, kCompactThreads, 4), kCompactThreads, 0,
                h->xi, h->v, h->cell, h->ctrl, h->tile_status);
-    SDM_LAUNCH(h, k_compact_finalize, 1, 1, 0, h->ctrl);
     h->stepped = false;                       // idx no longer refers to the current storage order
     return SDM_OK;
 }
@@ -319,6 +319,8 @@ int load_state_common(sdm_t *h, int64_t n_sd)
     // validation + layout analysis; synchronous
     Ctrl zero{};
     zero.n = (int)n_sd;
+    zero.epoch = 1;                                   // tile status words are tagged; 0 = never written
+    SDM_CUDA(h, cudaMemsetAsync(h->tile_status, 0, (size_t)h->L.n_tiles * 8, h->stream));
     SDM_CUDA(h, cudaMemcpyAsync(h->ctrl, &zero, sizeof(Ctrl), cudaMemcpyHostToDevice, h->stream));
     SDM_CUDA(h, cudaStreamSynchronize(h->stream));   // `zero` lives on this stack frame
     SDM_CUDA(h, cudaMemsetAsync(h->cell_cnt, 0, ((size_t)h->n_cell + 1) * 4, h->stream));
@@ -458,6 +460,10 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         h->sort_engine = (int)value;
         return SDM_OK;
     case SDM_OPT_SORT_FALLBACK: h->sort_fallback = value != 0; return SDM_OK;
+    case SDM_OPT_CTAS_PER_SM:
+        if (value < 0 || value > 32) return fail(h, SDM_EINVAL, "CTAs per SM: 0 (automatic) .. 32");
+        h->ctas_per_sm = (int)value;
+        return SDM_OK;
     default: return fail(h, SDM_EINVAL, "unknown option");
     }
 }

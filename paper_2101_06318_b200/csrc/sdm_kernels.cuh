@@ -24,7 +24,10 @@ struct Ctrl {
     int invalid;                   // analysis: validation failed
     int max_count;                 // analysis: largest cell
     unsigned int moment_done;      // moments: last-block counter
-    int pad0;
+    unsigned int compact_done;     // compaction: CTAs that have left the kernel
+    unsigned int epoch;            // compaction: tag of valid tile status words (no clearing between calls)
+    int cell_ticket;               // per-cell kernel: dynamic work counter
+    int pad0[2];
     unsigned long long n_events;   // pairs with gamma_tilde > 0
     unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
 };
@@ -419,7 +422,9 @@ k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ c
 // learns its output offset only after every earlier tile has published: so by the time a tile
 // writes into the (earlier) storage positions, everything there has been read.  Tiles are handed
 // out in order by a ticket, which guarantees forward progress of the look-back.
-constexpr unsigned long long kFlagAggregate = 1ull << 62, kFlagInclusive = 2ull << 62;
+// A tile status word is  epoch (30 bits) | flag (2 bits) | count (32 bits); words of earlier calls carry
+// an older epoch and read as "not published", so the array never has to be cleared.
+constexpr unsigned long long kFlagAggregate = 1ull << 32, kFlagInclusive = 2ull << 32;
 
 __global__ void __launch_bounds__(kCompactThreads)
 k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
@@ -432,6 +437,7 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
     __shared__ int s_tile, s_prefix;
     if (ctrl->zero_count == 0) return;                 // nothing to remove: every CTA leaves
     const int n = ctrl->n;
+    const unsigned long long tag = (unsigned long long)(ctrl->epoch & 0x3fffffffu) << 34;
     const int n_tiles = (n + kCompactTile - 1) / kCompactTile;
     const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
     constexpr int kItems = kCompactTile / kCompactThreads;      // 8
@@ -473,18 +479,18 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
             volatile unsigned long long *vs = status;
             __threadfence();
             if (tile == 0) {
-                vs[0] = kFlagInclusive | (unsigned long long)tile_total;
+                vs[0] = tag | kFlagInclusive | (unsigned long long)tile_total;
             } else {
-                vs[tile] = kFlagAggregate | (unsigned long long)tile_total;
+                vs[tile] = tag | kFlagAggregate | (unsigned long long)tile_total;
                 int t = tile - 1;
                 while (true) {
-                    unsigned long long st = vs[t];
-                    if ((st >> 62) == 0) continue;               // predecessor not published yet
+                    const unsigned long long st = vs[t];
+                    if ((st >> 34) != (tag >> 34) || ((st >> 32) & 3ull) == 0) continue;   // not published yet
                     excl += (int)(st & 0xffffffffull);
-                    if ((st >> 62) == 2) break;
+                    if (((st >> 32) & 3ull) == 2) break;
                     --t;
                 }
-                vs[tile] = kFlagInclusive | (unsigned long long)(excl + tile_total);
+                vs[tile] = tag | kFlagInclusive | (unsigned long long)(excl + tile_total);
             }
             __threadfence();
             s_prefix = excl;
@@ -505,13 +511,20 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
             run += __popc(masks[k]);
         }
     }
-}
-
-__global__ void k_compact_finalize(Ctrl *ctrl)
-{
-    if (ctrl->zero_count > 0) ctrl->n = ctrl->n_new;
-    ctrl->zero_count = 0;
-    ctrl->ticket = 0;
+    // the last CTA to leave publishes the new count and re-arms the control block; every CTA has read
+    // zero_count and n before it counts itself out, so nobody sees the new values half-way
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(&ctrl->compact_done, 1u) == gridDim.x - 1) {
+            __threadfence();
+            ctrl->n = ((volatile Ctrl *)ctrl)->n_new;
+            ctrl->zero_count = 0;
+            ctrl->ticket = 0;
+            ctrl->compact_done = 0;
+            ctrl->epoch = ctrl->epoch + 1u;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
