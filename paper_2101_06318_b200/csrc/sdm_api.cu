@@ -214,7 +214,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
 {
     const int64_t n_ub = h->n_ub;
     if (use_fused(h)) {
-        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 3) / 4, 256, 32), 256, 0, h->cell, h->ctrl, h->n_cell,
+        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 4 * kCellStartQuads - 1) / (4 * kCellStartQuads), 256, 32), 256, 0, h->cell, h->ctrl, h->n_cell,
                    h->cell_start);
         // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
         // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose

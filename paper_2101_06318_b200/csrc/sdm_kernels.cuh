@@ -12,6 +12,7 @@ constexpr int kCompactTile = 2048;       // elements per compaction tile
 constexpr int kCompactThreads = 256;
 constexpr int kMomentBlocks = 1184;      // 148 SMs x 8
 constexpr int kMomentThreads = 256;
+constexpr int kCellStartQuads = 4;       // k_cell_start_sorted: 16-byte loads per thread and round
 
 // Device-resident control block: everything the host would otherwise have to synchronise for.
 struct Ctrl {
@@ -389,28 +390,54 @@ k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ c
     }
     const int n4 = (n + 3) >> 2;
     const int4 *cell4 = reinterpret_cast<const int4 *>(cell);
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += gridDim.x * blockDim.x) {
-        const int i = t << 2;
-        int c0, c1, c2, c3;
-        if (i + 3 < n) {
-            const int4 q = __ldcs(cell4 + t);
-            c0 = q.x; c1 = q.y; c2 = q.z; c3 = q.w;
-        } else {
-            c0 = cell[i];
-            c1 = (i + 1 < n) ? cell[i + 1] : c0;
-            c2 = (i + 2 < n) ? cell[i + 2] : c1;
-            c3 = c2;
+    const int T = blockDim.x, lane = lane_id();                     // a CTA reads U*T consecutive quads per round
+    constexpr int U = kCellStartQuads;                              // independent 16-byte loads in flight per thread
+    for (int t0 = blockIdx.x * (U * T) + threadIdx.x; t0 - lane < n4; t0 += gridDim.x * (U * T)) {
+        const int t_hi = t0 - lane + 31 + (U - 1) * T;              // the largest quad index this warp touches
+        if (t_hi < n4 - 1 && t0 - lane > 0) {
+            // fast path (warp-uniform): every quad is complete and none is the first or the last
+            int4 q[U];
+            int pv[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) q[u] = __ldcs(cell4 + t0 + u * T);
+#pragma unroll
+            for (int u = 0; u < U; ++u) pv[u] = (lane == 0) ? __ldg(cell + ((t0 + u * T) << 2) - 1) : 0;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = (t0 + u * T) << 2;
+                int prev = __shfl_up_sync(0xffffffffu, q[u].w, 1);  // the droplet before this thread's four
+                if (lane == 0) prev = pv[u];
+                if (prev != q[u].w) {                               // some boundary among the four
+                    if (q[u].x != prev) cell_boundary(prev, q[u].x, i, cell_start);
+                    if (q[u].y != q[u].x) cell_boundary(q[u].x, q[u].y, i + 1, cell_start);
+                    if (q[u].z != q[u].y) cell_boundary(q[u].y, q[u].z, i + 2, cell_start);
+                    if (q[u].w != q[u].z) cell_boundary(q[u].z, q[u].w, i + 3, cell_start);
+                }
+            }
+            continue;
         }
-        const int prev = (i > 0) ? __ldg(cell + i - 1) : -1;
-        if (prev != c3) {                                           // some boundary among the four
-            if (c0 != prev) cell_boundary(prev, c0, i, cell_start);
-            if (c1 != c0) cell_boundary(c0, c1, i + 1, cell_start);
-            if (c2 != c1) cell_boundary(c1, c2, i + 2, cell_start);
-            if (c3 != c2) cell_boundary(c2, c3, i + 3, cell_start);
-        }
-        if (i + 4 >= n) {                                           // the thread holding the last droplet
-            const int last = (i + 3 < n) ? c3 : ((i + 2 < n) ? c2 : ((i + 1 < n) ? c1 : c0));
-            for (int cc = last + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
+        for (int u = 0; u < U; ++u) {                               // edges of the array
+            const int t = t0 + u * T, i = t << 2;
+            if (t >= n4) break;
+            int c0, c1, c2, c3;
+            if (i + 3 < n) {
+                const int4 q = __ldcs(cell4 + t);
+                c0 = q.x; c1 = q.y; c2 = q.z; c3 = q.w;
+            } else {                                                // the last, partial quad: repeat the last id
+                c0 = cell[i];
+                c1 = (i + 1 < n) ? cell[i + 1] : c0;
+                c2 = (i + 2 < n) ? cell[i + 2] : c1;
+                c3 = c2;
+            }
+            const int prev = (i > 0) ? __ldg(cell + i - 1) : -1;
+            if (prev != c3) {
+                if (c0 != prev) cell_boundary(prev, c0, i, cell_start);
+                if (c1 != c0) cell_boundary(c0, c1, i + 1, cell_start);
+                if (c2 != c1) cell_boundary(c1, c2, i + 2, cell_start);
+                if (c3 != c2) cell_boundary(c2, c3, i + 3, cell_start);
+            }
+            if (i + 4 >= n)                                         // the thread holding the last droplet
+                for (int cc = c3 + 1; cc <= n_cell; ++cc) cell_start[cc] = n;
         }
     }
 }
