@@ -44,6 +44,22 @@ def measured_peak_gbs():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+def ncu_dram_bytes(path):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the first captured launch in an ncu summary csv."""
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total, seen = 0.0, 0
+    try:
+        with open(path) as f:
+            for line in f:
+                parts = line.strip().split(",")
+                if parts[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    total += float(parts[2]) * scale[parts[1]]
+                    seen += 1
+    except Exception:
+        return None
+    return total if seen == 2 else None
+
+
 def build_workload(name: str, rank: int = 0, scale_cells: int | None = None):
     import workloads
     if name == "C5":
@@ -318,15 +334,9 @@ def main():
             roofline = {"bound": "hbm", "kernel": "k_segment_sort (general path; L2-resident workload)",
                         "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
                         "ms_per_launch": per_launch_s * 1e3, "launches_timed": kernel_n}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic_fused_kernel.json")
-    if roofline is not None and mode == 1 and os.path.exists(traffic_file):
-        try:
-            with open(traffic_file) as f:
-                tf = json.load(f)
-            if tf.get("n_sd") == w.n_sd:
-                roofline["traffic"] = tf.get("dram_bytes_per_launch")
-        except Exception:
-            pass
+    # traffic: DRAM bytes per launch of the dominant kernel from the committed ncu summary (C5 only)
+    if roofline is not None and mode == 1 and w.n_sd == 67108864:
+        roofline["traffic"] = ncu_dram_bytes(os.path.join(ROOT, "profiles", "r01_ncu_fused_kernel_c5.csv"))
 
     cpu = None
     if not args.no_cpu_baseline:
