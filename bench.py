@@ -243,9 +243,12 @@ def main():
     mode = s.counters()["mode"]
     mom = s.moments()
 
+    from paper_2101_06318_b200 import sharding
+    seed = sharding.shard_seed(w.seed, rank)     # every rank owns its cells and its own Philox key
+
     def one_step(step):
         s.remove_zero(sync=False)
-        s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step, out=mom)
+        s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, seed, step, out=mom)
 
     def barrier():
         if dist is not None:
