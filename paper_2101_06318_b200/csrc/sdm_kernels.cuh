@@ -43,15 +43,22 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
                           int *__restrict__ cell_cnt, Ctrl *ctrl)
 {
     int zeros = 0, bad = 0, unsorted = 0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        int c = cell[i];
-        int64_t x = xi[i];
-        double vol = v[i];
-        bool ok = (c >= 0) && (c < n_cell) && (x >= 0) && (vol > 0.0) && (vol < CUDART_INF);
-        if (!ok) { bad = 1; continue; }
-        zeros += (x == 0);
-        if (i > 0 && cell[i - 1] > c) unsorted = 1;
-        atomicAdd(&cell_cnt[c], 1);
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane_id();
+        int c = -1;
+        if (i < n) {
+            c = cell[i];
+            const int64_t x = xi[i];
+            const double vol = v[i];
+            const bool ok = (c >= 0) && (c < n_cell) && (x >= 0) && (vol > 0.0) && (vol < CUDART_INF);
+            if (!ok) { bad = 1; c = -1; }
+            else {
+                zeros += (x == 0);
+                if (i > 0 && cell[i - 1] > c) unsorted = 1;
+            }
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, c);   // one atomic per distinct cell and warp
+        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(&cell_cnt[c], __popc(peers));
     }
     zeros = __reduce_add_sync(0xffffffffu, zeros);
     bad = __any_sync(0xffffffffu, bad);
@@ -79,8 +86,13 @@ __global__ void k_cell_count(const int32_t *__restrict__ cell, const Ctrl *__res
                              int *__restrict__ cell_cnt)
 {
     const int n = ctrl->n;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-        atomicAdd(&cell_cnt[cell[i]], 1);
+    // lanes of a warp that hit the same cell (all of them in a single-cell box) send ONE atomic
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane_id();
+        const int c = (i < n) ? cell[i] : -1;
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
+        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(&cell_cnt[c], __popc(peers));
+    }
 }
 
 // Single-CTA exclusive scan of per-cell counts -> cell_start[n_cell+1].  With split != 0 it also
