@@ -16,6 +16,7 @@
 #include "sdm_kernels.cuh"
 #include "sdm_fused.cuh"
 #include "sdm_fused_count.cuh"
+#include "sdm_general.cuh"
 
 using namespace sdmk;
 
@@ -92,7 +93,8 @@ struct sdm {
     int num_sms = 148;
     // options
     bool force_general = false;
-    int seg_cap = kWarpCap;
+    int seg_cap = kWarpCap;      // fused path: largest cell; general path: only when overridden (tests)
+    bool seg_cap_set = false;    // SDM_OPT_SEGMENT_CAP given: general path sorts with the bitonic kernel
     bool write_idx = true;
     bool screening = true;
     int lanes_per_cell = 0;      // 0: automatic
@@ -171,6 +173,9 @@ bool use_fused(const sdm_t *h)
 {
     return h->sorted && !h->force_general && h->max_count <= h->seg_cap && h->max_count <= 512;
 }
+
+// largest segment of the general path: the warp counting sort holds 256 droplets
+int general_cap(const sdm_t *h) { return h->seg_cap_set ? h->seg_cap : kGenCap; }
 
 constexpr size_t kSortSmem = (size_t)kSortWarps * kWarpCap * (sizeof(uint64_t) + sizeof(int));
 
@@ -260,12 +265,14 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
 #undef SDM_FUSED
         return SDM_OK;
     }
-    const bool split = h->max_count > h->seg_cap;
+    const int gcap = general_cap(h);
+    const bool split = h->max_count > gcap;
     const int g = grid_for(h, n_ub, 256, 16);
     SDM_CUDA(h, cudaMemsetAsync(h->cell_cnt, 0, ((size_t)h->n_cell + 1) * 4, h->stream));
-    SDM_LAUNCH(h, k_cell_count, g, 256, 0, h->cell, h->ctrl, h->cell_cnt);
+    SDM_LAUNCH(h, k_cell_count, h->n_cell <= kCellCountBins ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell, h->ctrl,
+               h->n_cell, h->cell_cnt);
     SDM_LAUNCH(h, k_cell_scan, 1, kScanThreads, 0, h->cell_cnt, h->n_cell, h->cell_start, split ? 1 : 0,
-               h->seg_cap, h->cell_bits, h->bucket_base, h->ctrl);
+               gcap, h->cell_bits, h->bucket_base, h->ctrl);
     const int *seg_start = h->cell_start;
     int n_seg_host = h->n_cell;
     int *cursor = h->cell_cnt;
@@ -284,9 +291,14 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     SDM_LAUNCH(h, k_scatter, g, 256, 0, h->cell, h->ctrl, split ? 1 : 0, h->cell_bits, h->bucket_base,
                seg_start, cursor, h->order, prm.seed, prm.step);
     int64_t seg_ub = split ? h->L.nb_max : (int64_t)h->n_cell;
-    SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort, grid_for(h, seg_ub * 32, kSortWarps * 32, 4), kSortWarps * 32,
-                            kSortSmem, seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed,
-                            prm.step));
+    if (h->seg_cap_set)
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort, grid_for(h, seg_ub * 32, kSortWarps * 32, 4), kSortWarps * 32,
+                                kSortSmem, seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed,
+                                prm.step));
+    else
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_count, grid_for(h, seg_ub * 32, kGenWarps * 32, 3), kGenWarps * 32,
+                                kGenSmemBytes, seg_start, h->ctrl, n_seg_host, h->order, h->cell, h->cell_bits,
+                                h->idx, prm));
     SDM_LAUNCH(h, k_pairs_by_position, g, 256, 0, h->xi, h->v, h->cell, h->idx, h->cell_start, h->ctrl, prm);
     if (m0) return enqueue_moments(h, 0, m0, m1, m2);
     return SDM_OK;
@@ -412,6 +424,8 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
     e = cudaFuncSetAttribute(k_segment_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort)");
+    e = cudaFuncSetAttribute(k_segment_sort_count, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_count)");
     e = cudaFuncSetAttribute(k_fused_cells_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<true>)");
     e = cudaFuncSetAttribute(k_fused_cells_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
@@ -442,11 +456,12 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
     switch (option) {
     case SDM_OPT_FORCE_GENERAL: h->force_general = value != 0; return SDM_OK;
     case SDM_OPT_SEGMENT_CAP:
-        if (value == 0) { h->seg_cap = kWarpCap; return SDM_OK; }
+        if (value == 0) { h->seg_cap = kWarpCap; h->seg_cap_set = false; return SDM_OK; }
         if (value < kMinSegCap || value > kWarpCap) return fail(h, SDM_EINVAL, "segment cap must be in [8, 512]");
         if ((int64_t)h->n_cell + 4 * h->capacity / value + 2 > h->L.nb_max)
             return fail(h, SDM_EINVAL, "segment cap too small for this workspace");
         h->seg_cap = (int)value;
+        h->seg_cap_set = true;
         return SDM_OK;
     case SDM_OPT_WRITE_IDX: h->write_idx = value != 0; return SDM_OK;
     case SDM_OPT_SCREENING: h->screening = value != 0; return SDM_OK;

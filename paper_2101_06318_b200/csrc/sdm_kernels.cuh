@@ -82,16 +82,30 @@ __global__ void k_max_count(const int *__restrict__ cell_cnt, int n_cell, Ctrl *
 // ---------------------------------------------------------------------------------------------
 // Row a2 (general path): counting sort by cell -- histogram, scan, scatter
 // ---------------------------------------------------------------------------------------------
-__global__ void k_cell_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
-                             int *__restrict__ cell_cnt)
+constexpr int kCellCountBins = 2048;     // up to this many cells the histogram is privatised per CTA
+
+__global__ void __launch_bounds__(256)
+k_cell_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell,
+             int *__restrict__ cell_cnt)
 {
+    __shared__ int s_cnt[kCellCountBins];
     const int n = ctrl->n;
+    const bool priv = n_cell <= kCellCountBins;       // few cells (a box is ONE cell): same-address atomics
+    if (priv) {                                       // would serialise in L2, so count in shared memory first
+        for (int c = threadIdx.x; c < n_cell; c += blockDim.x) s_cnt[c] = 0;
+        __syncthreads();
+    }
     // lanes of a warp that hit the same cell (all of them in a single-cell box) send ONE atomic
     for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
         const int i = i0 + lane_id();
         const int c = (i < n) ? cell[i] : -1;
         const unsigned peers = __match_any_sync(0xffffffffu, c);
-        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(&cell_cnt[c], __popc(peers));
+        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(priv ? &s_cnt[c] : &cell_cnt[c], __popc(peers));
+    }
+    if (priv) {
+        __syncthreads();
+        for (int c = threadIdx.x; c < n_cell; c += blockDim.x)
+            if (s_cnt[c]) atomicAdd(&cell_cnt[c], s_cnt[c]);
     }
 }
 
