@@ -94,7 +94,10 @@ struct sdm {
     // options
     bool force_general = false;
     int seg_cap = kWarpCap;      // fused path: largest cell; general path: only when overridden (tests)
-    bool seg_cap_set = false;    // SDM_OPT_SEGMENT_CAP given: general path sorts with the bitonic kernel
+    bool seg_cap_set = false;    // SDM_OPT_SEGMENT_CAP given
+    bool tables_ready = false;   // general path: cell_bits / bucket_base / n_seg are valid for this state
+    bool split = false;          // general path: some cell is larger than a sort segment
+    int n_seg = 0;               // general path: number of sort segments when split
     bool write_idx = true;
     bool screening = true;
     int lanes_per_cell = 0;      // 0: automatic
@@ -177,7 +180,6 @@ bool use_fused(const sdm_t *h)
 // largest segment of the general path: the warp counting sort holds 256 droplets
 int general_cap(const sdm_t *h) { return h->seg_cap_set ? h->seg_cap : kGenCap; }
 
-constexpr size_t kSortSmem = (size_t)kSortWarps * kWarpCap * (sizeof(uint64_t) + sizeof(int));
 
 int read_ctrl(sdm_t *h)
 {
@@ -207,6 +209,24 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.screening = h->screening ? 1 : 0;
     prm.sort_fallback = h->sort_fallback ? 1 : 0;
     philox_round_keys(seed, prm.rk);
+    return SDM_OK;
+}
+
+// General path: the static split of large cells into sort segments (cell_bits, bucket_base, n_seg), decided
+// from the current cell counts; SYNCHRONOUS (reads n_seg back), done once per loaded state / option change.
+int build_tables(sdm_t *h)
+{
+    const int gcap = general_cap(h);
+    h->split = h->max_count > gcap;
+    SDM_LAUNCH(h, k_cell_count, h->n_cell <= kCellCountBins ? grid_for(h, h->n_ub, 256, 4) : grid_for(h, h->n_ub, 256, 16),
+               256, 0, h->cell, h->ctrl, h->n_cell, h->cell_cnt);
+    SDM_LAUNCH(h, k_cell_scan, 1, kScanThreads, 0, h->cell_cnt, h->n_cell, h->cell_start, h->split ? 1 : 0, gcap,
+               h->cell_bits, h->bucket_base, h->ctrl);
+    int rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    h->n_seg = h->ctrl_host->n_buckets;
+    if (h->n_seg > h->L.nb_max) return fail(h, SDM_EINVAL, "segment table exceeds the workspace (segment cap too small)");
+    h->tables_ready = true;
     return SDM_OK;
 }
 
@@ -265,41 +285,26 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
 #undef SDM_FUSED
         return SDM_OK;
     }
-    const int gcap = general_cap(h);
-    const bool split = h->max_count > gcap;
-    const int g = grid_for(h, n_ub, 256, 16);
-    SDM_CUDA(h, cudaMemsetAsync(h->cell_cnt, 0, ((size_t)h->n_cell + 1) * 4, h->stream));
-    SDM_LAUNCH(h, k_cell_count, h->n_cell <= kCellCountBins ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell, h->ctrl,
-               h->n_cell, h->cell_cnt);
-    SDM_LAUNCH(h, k_cell_scan, 1, kScanThreads, 0, h->cell_cnt, h->n_cell, h->cell_start, split ? 1 : 0,
-               gcap, h->cell_bits, h->bucket_base, h->ctrl);
-    const int *seg_start = h->cell_start;
-    int n_seg_host = h->n_cell;
-    int *cursor = h->cell_cnt;
-    size_t cursor_bytes = ((size_t)h->n_cell + 1) * 4;
-    if (split) {
-        SDM_CUDA(h, cudaMemsetAsync(h->bucket_cnt, 0, ((size_t)h->L.nb_max + 1) * 4, h->stream));
-        SDM_LAUNCH(h, k_bucket_count, g, 256, 0, h->cell, h->ctrl, h->cell_bits, h->bucket_base, h->bucket_cnt,
-                   prm.seed, prm.step);
-        SDM_LAUNCH(h, k_bucket_scan, 1, kScanThreads, 0, h->bucket_cnt, h->ctrl, h->bucket_start);
-        seg_start = h->bucket_start;
-        n_seg_host = -1;                      // number of buckets is on the device
-        cursor = h->bucket_cnt;
-        cursor_bytes = ((size_t)h->L.nb_max + 1) * 4;
+    if (!h->tables_ready) {
+        int rc = build_tables(h);
+        if (rc != SDM_OK) return rc;
     }
-    SDM_CUDA(h, cudaMemsetAsync(cursor, 0, cursor_bytes, h->stream));
-    SDM_LAUNCH(h, k_scatter, g, 256, 0, h->cell, h->ctrl, split ? 1 : 0, h->cell_bits, h->bucket_base,
-               seg_start, cursor, h->order, prm.seed, prm.step);
-    int64_t seg_ub = split ? h->L.nb_max : (int64_t)h->n_cell;
-    if (h->seg_cap_set)
-        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort, grid_for(h, seg_ub * 32, kSortWarps * 32, 4), kSortWarps * 32,
-                                kSortSmem, seg_start, h->ctrl, n_seg_host, h->seg_cap, h->order, h->idx, prm.seed,
-                                prm.step));
-    else
-        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_count, grid_for(h, seg_ub * 32, kGenWarps * 32, 3), kGenWarps * 32,
-                                kGenSmemBytes, seg_start, h->ctrl, n_seg_host, h->order, h->cell, h->cell_bits,
-                                h->idx, prm));
-    SDM_LAUNCH(h, k_pairs_by_position, g, 256, 0, h->xi, h->v, h->cell, h->idx, h->cell_start, h->ctrl, prm);
+    const int split = h->split ? 1 : 0;
+    const int n_seg = split ? h->n_seg : h->n_cell;
+    int *seg_start = split ? h->bucket_start : h->cell_start;
+    const int g = grid_for(h, n_ub, 256, 16);
+    SDM_LAUNCH(h, k_gen_count, h->n_cell <= kCellCountBins ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell, h->ctrl,
+               h->n_cell, split, h->cell_bits, h->bucket_base, h->cell_cnt, h->bucket_cnt, prm);
+    SDM_LAUNCH(h, k_gen_scan, 1, kScanThreads, 0, h->cell_cnt, h->n_cell, h->cell_start, split, h->bucket_cnt,
+               n_seg, h->bucket_start);
+    SDM_LAUNCH(h, k_gen_scatter, g, 256, 0, h->cell, h->ctrl, split, h->cell_bits, h->bucket_base, seg_start,
+               h->bucket_cnt, h->order, prm);
+    SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
+                            kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
+                            h->cell, h->cell_bits, h->cell_start, h->bucket_cnt, h->idx, h->xi, h->v, h->ctrl, prm));
+    if (split)
+        SDM_LAUNCH(h, k_pairs_straddle, grid_for(h, n_seg, 256, 8), 256, 0, seg_start, n_seg, h->idx, h->cell,
+                   h->cell_start, h->xi, h->v, h->ctrl, prm);
     if (m0) return enqueue_moments(h, 0, m0, m1, m2);
     return SDM_OK;
 }
@@ -349,6 +354,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
                     "state validation failed: need 0 <= cell_id < n_cell, xi >= 0, v finite and > 0");
     }
     h->valid = true;
+    h->tables_ready = false;
     h->n_ub = n_sd;
     h->max_count = h->ctrl_host->max_count;
     h->sorted = (h->ctrl_host->unsorted == 0);
@@ -422,16 +428,18 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     };
     e = cudaMallocHost(reinterpret_cast<void **>(&h->ctrl_host), sizeof(Ctrl));
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
-    e = cudaFuncSetAttribute(k_segment_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort)");
-    e = cudaFuncSetAttribute(k_segment_sort_count, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_count)");
+    e = cudaFuncSetAttribute(k_segment_sort_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_pairs)");
     e = cudaFuncSetAttribute(k_fused_cells_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<true>)");
     e = cudaFuncSetAttribute(k_fused_cells_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<false>)");
     e = cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(ctrl)");
+    e = cudaMemsetAsync(h->cell_cnt, 0, ((size_t)n_cell + 1) * 4, h->stream);
+    if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(cell_cnt)");
+    e = cudaMemsetAsync(h->bucket_cnt, 0, ((size_t)h->L.nb_max + 1) * 4, h->stream);
+    if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(bucket_cnt)");
     e = cudaMemsetAsync(h->cell_start, 0, ((size_t)n_cell + 1) * 4, h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(cell_start)");
     e = cudaStreamSynchronize(h->stream);
@@ -454,10 +462,11 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
 {
     if (!h) return SDM_EINVAL;
     switch (option) {
-    case SDM_OPT_FORCE_GENERAL: h->force_general = value != 0; return SDM_OK;
+    case SDM_OPT_FORCE_GENERAL: h->force_general = value != 0; h->tables_ready = false; return SDM_OK;
     case SDM_OPT_SEGMENT_CAP:
+        h->tables_ready = false;
         if (value == 0) { h->seg_cap = kWarpCap; h->seg_cap_set = false; return SDM_OK; }
-        if (value < kMinSegCap || value > kWarpCap) return fail(h, SDM_EINVAL, "segment cap must be in [8, 512]");
+        if (value < kMinSegCap || value > kGenCap) return fail(h, SDM_EINVAL, "segment cap must be in [8, 256]");
         if ((int64_t)h->n_cell + 4 * h->capacity / value + 2 > h->L.nb_max)
             return fail(h, SDM_EINVAL, "segment cap too small for this workspace");
         h->seg_cap = (int)value;

@@ -104,13 +104,138 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[8], int m, int la
     }
 }
 
-// seg_start[0..n_seg]: segment boundaries in order[]; n_seg_host < 0: the number of segments is
-// ctrl->n_buckets (split mode), and cell_bits[cell] gives the key bits a segment's droplets share.
+// ---------------------------------------------------------------------------------------------
+// Per-step pipeline of the general path:  k_gen_count -> k_gen_scan -> k_gen_scatter ->
+// k_segment_sort_pairs (-> k_pairs_straddle when cells are split).
+//
+// The split of large cells (cell_bits[c] = B key bits, bucket_base[c] = first segment of cell c) is
+// decided ONCE per loaded state from the cell counts (k_cell_scan with split = 1): cells never grow
+// (PAPER.md:9, 77), so the segments only get smaller afterwards, and idx does not depend on B.
+// Invariant between steps: cell_cnt[] and seg_cnt[] are all zero (every consumer clears what it read).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int segment_of(int c, uint32_t key_hi, const int *__restrict__ cell_bits,
+                                          const int *__restrict__ bucket_base)
+{
+    const int B = cell_bits[c];
+    return bucket_base[c] + (B > 0 ? (int)(key_hi >> (32 - B)) : 0);
+}
+
+// Row a2: per-cell counts (warp-aggregated; CTA-privatised when there are few cells) and, when cells
+// are split, per-segment counts (needs the droplet's Philox block, row a1).
+__global__ void __launch_bounds__(256)
+k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell, int split,
+            const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
+            int *__restrict__ cell_cnt, int *__restrict__ seg_cnt, const __grid_constant__ StepParams prm)
+{
+    __shared__ int s_cnt[kCellCountBins];
+    const int n = ctrl->n;
+    const bool priv = n_cell <= kCellCountBins;
+    if (priv) {
+        for (int c = threadIdx.x; c < n_cell; c += blockDim.x) s_cnt[c] = 0;
+        __syncthreads();
+    }
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane_id();
+        const int c = (i < n) ? cell[i] : -1;
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
+        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(priv ? &s_cnt[c] : &cell_cnt[c], __popc(peers));
+        if (split && c >= 0) {
+            const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
+            atomicAdd(&seg_cnt[segment_of(c, w.y, cell_bits, bucket_base)], 1);
+        }
+    }
+    if (priv) {
+        __syncthreads();
+        for (int c = threadIdx.x; c < n_cell; c += blockDim.x)
+            if (s_cnt[c]) atomicAdd(&cell_cnt[c], s_cnt[c]);
+    }
+}
+
+// Exclusive scans: cell counts -> cell_start[n_cell+1] and (split) segment counts -> seg_start[n_seg+1].
+// Clears the counters it reads.  One CTA.
+__global__ void __launch_bounds__(kScanThreads)
+k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start, int split,
+           int *__restrict__ seg_cnt, int n_seg, int *__restrict__ seg_start)
+{
+    __shared__ int s_warp[33];
+    for (int pass = 0; pass < (split ? 2 : 1); ++pass) {
+        int *cnt = pass ? seg_cnt : cell_cnt;
+        int *start = pass ? seg_start : cell_start;
+        const int m = pass ? n_seg : n_cell;
+        int carry = 0;
+        for (int base = 0; base < m; base += kScanThreads * kScanItems) {
+            const int c0 = base + threadIdx.x * kScanItems;
+            int loc[kScanItems];
+            int sum = 0;
+#pragma unroll
+            for (int k = 0; k < kScanItems; ++k) {
+                loc[k] = (c0 + k < m) ? cnt[c0 + k] : 0;
+                sum += loc[k];
+            }
+            int total;
+            int run = carry + block_exclusive_scan(sum, s_warp, total);
+#pragma unroll
+            for (int k = 0; k < kScanItems; ++k) {
+                if (c0 + k < m) { start[c0 + k] = run; cnt[c0 + k] = 0; }
+                run += loc[k];
+            }
+            carry += total;
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) start[m] = carry;
+        __syncthreads();
+    }
+}
+
+// order[] = storage indices grouped by segment (arbitrary order inside; the sort makes it unique).
+// cursor[] must be zero on entry; the sort kernel clears it again.
+__global__ void __launch_bounds__(256)
+k_gen_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int split,
+              const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
+              const int *__restrict__ seg_start, int *__restrict__ cursor, int *__restrict__ order,
+              const __grid_constant__ StepParams prm)
+{
+    const int n = ctrl->n;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int c = cell[i];
+        int b = c;
+        if (split) {
+            const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
+            b = segment_of(c, w.y, cell_bits, bucket_base);
+        }
+        const int pos = atomicAdd(&cursor[b], 1);
+        order[seg_start[b] + pos] = i;
+    }
+}
+
+// Rows a4-a6 for the candidate pairs that lie inside one sorted segment [s, s+m) of the cell that
+// starts at cs and holds n_s droplets (Fig. 4: positions cs+2k, cs+2k+1 pair up).
+// sorted[e] = storage index at position s+e.  A pair whose second member is the first droplet of the
+// next segment is left to k_pairs_straddle.  Returns events | zeros << 10 | exact << 20 of this lane.
+__device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, int cs, int n_s, int lane,
+                                             int64_t *__restrict__ xi, double *__restrict__ v,
+                                             const StepParams &prm)
+{
+    const double norm = pair_norm(n_s, prm.dtdv);
+    int packed = 0;
+    for (int e = ((s - cs) & 1) + 2 * lane; e + 1 < m; e += 64) {
+        const int a = sorted[e], b = sorted[e + 1];
+        const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
+        const int r = collide_pair_exact(xi, v, a, b, u, norm, prm.kernel, prm.kparam);
+        packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
+    }
+    return packed;
+}
+
+// seg_start[0..n_seg]: segment boundaries in order[]; split != 0: segments are pieces of cells and
+// cell_bits[cell] gives the key bits a segment's droplets share.  seg_cap <= 256: larger segments are
+// ranked by counting (tests lower it).  Clears cursor[seg].
 __global__ void __launch_bounds__(kGenWarps * 32)
-k_segment_sort_count(const int *__restrict__ seg_start, const Ctrl *__restrict__ ctrl, int n_seg_host,
+k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, int seg_cap,
                      const int *__restrict__ order, const int32_t *__restrict__ cell,
-                     const int *__restrict__ cell_bits, int *__restrict__ idx,
-                     const __grid_constant__ StepParams prm)
+                     const int *__restrict__ cell_bits, const int *__restrict__ cell_start,
+                     int *__restrict__ cursor, int *__restrict__ idx, int64_t *__restrict__ xi,
+                     double *__restrict__ v, Ctrl *ctrl, const __grid_constant__ StepParams prm)
 {
     constexpr int E = 8, L = 32, N = kGenCap;
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
@@ -121,64 +246,114 @@ k_segment_sort_count(const int *__restrict__ seg_start, const Ctrl *__restrict__
     const PhiloxKey &rk = prm.rk;
     for (int i = lane; i < 256; i += 32) sm->cnt[i] = 0;
     __syncwarp();
-    const bool split = n_seg_host < 0;
-    const int n_seg = split ? ctrl->n_buckets : n_seg_host;
+    int packed_sum_ev = 0, packed_sum_z = 0, packed_sum_ex = 0;
     const int warps_total = gridDim.x * kGenWarps;
     for (int seg = blockIdx.x * kGenWarps + (threadIdx.x >> 5); seg < n_seg; seg += warps_total) {
         const int s = seg_start[seg];
         const int m = seg_start[seg + 1] - s;
         if (m == 0) continue;
-        if (m > N) {
+        if (lane == 0) cursor[seg] = 0;
+        const int id0 = order[s];
+        const int c = cell[id0];
+        const int cs = cell_start[c], n_s = cell_start[c + 1] - cs;
+        int pk;
+        if (m > seg_cap) {
             warp_rank_by_counting(order + s, 0, m, s, idx, prm.step, rk, lane);
-            continue;
-        }
-        if (m == 1) {
-            if (lane == 0) idx[s] = order[s];
-            continue;
-        }
-        const int nrem = m - lane;
-        int id[E];
+            __threadfence_block();
+            __syncwarp();
+            pk = segment_pairs(idx + s, s, m, cs, n_s, lane, xi, v, prm);
+        } else if (m == 1) {
+            if (lane == 0) idx[s] = id0;
+            pk = 0;
+        } else {
+            const int nrem = m - lane;
+            int id[E];
 #pragma unroll
-        for (int k = 0; k < E; ++k) {
-            id[k] = (nrem > L * k) ? order[s + lane + L * k] : 0;
-            sm->ids[lane + L * k] = id[k];
-        }
-        int shift = 0;
-        if (split) shift = cell_bits[cell[__shfl_sync(0xffffffffu, id[0], 0)]];
-        uint32_t x[E];
-        count_sort_ids(id, m, lane, shift, prm.step, rk, sm, sm_base, x);
-        // adjacent words that share the truncated key differ by less than N
-        const uint32_t nx0 = __shfl_down_sync(0xffffffffu, x[0], 1);
-        uint32_t dmin = 0xFFFFFFFFu;
-        const int l0 = m - E * lane;                      // position 8*lane + r exists iff r < l0
-#pragma unroll
-        for (int r = 0; r + 1 < E; ++r)
-            if (l0 > r + 1) dmin = min(dmin, x[r + 1] - x[r]);
-        if (l0 > E) dmin = min(dmin, nx0 - x[E - 1]);
-        if (__any_sync(0xffffffffu, dmin < (uint32_t)N)) {
-            // exact path: bitonic network on (key64, storage index), R7
-            int P = 2;
-            while (P < m) P <<= 1;
-            for (int e = lane; e < P; e += 32) {
-                if (e < m) {
-                    const int d = sm->ids[e];
-                    sm->key[e] = block_key64(droplet_block((uint32_t)d, prm.step, rk));
-                    sm->sid[e] = d;
-                } else {
-                    sm->key[e] = ~0ull;
-                    sm->sid[e] = 0x7fffffff;
-                }
+            for (int k = 0; k < E; ++k) {
+                id[k] = (nrem > L * k) ? order[s + lane + L * k] : 0;
+                sm->ids[lane + L * k] = id[k];
             }
-            __syncwarp();
-            warp_bitonic(sm->key, sm->sid, P, lane);
-            for (int e = lane; e < m; e += 32) idx[s + e] = sm->sid[e];
-            __syncwarp();
-            continue;
-        }
+            const int shift = split ? cell_bits[c] : 0;
+            uint32_t x[E];
+            count_sort_ids(id, m, lane, shift, prm.step, rk, sm, sm_base, x);
+            // adjacent words that share the truncated key differ by less than N
+            const uint32_t nx0 = __shfl_down_sync(0xffffffffu, x[0], 1);
+            uint32_t dmin = 0xFFFFFFFFu;
+            const int l0 = m - E * lane;                  // position 8*lane + r exists iff r < l0
 #pragma unroll
-        for (int r = 0; r < E; ++r)
-            if (l0 > r) idx[s + E * lane + r] = sm->ids[x[r] & (N - 1)];
-        __syncwarp();                                     // ids[] and slot[] are rewritten by the next segment
+            for (int r = 0; r + 1 < E; ++r)
+                if (l0 > r + 1) dmin = min(dmin, x[r + 1] - x[r]);
+            if (l0 > E) dmin = min(dmin, nx0 - x[E - 1]);
+            if (__any_sync(0xffffffffu, dmin < (uint32_t)N)) {
+                // exact path: bitonic network on (key64, storage index), R7
+                int P = 2;
+                while (P < m) P <<= 1;
+                for (int e = lane; e < P; e += 32) {
+                    if (e < m) {
+                        const int d = sm->ids[e];
+                        sm->key[e] = block_key64(droplet_block((uint32_t)d, prm.step, rk));
+                        sm->sid[e] = d;
+                    } else {
+                        sm->key[e] = ~0ull;
+                        sm->sid[e] = 0x7fffffff;
+                    }
+                }
+                __syncwarp();
+                warp_bitonic(sm->key, sm->sid, P, lane);
+            } else {
+#pragma unroll
+                for (int r = 0; r < E; ++r)
+                    if (l0 > r) sm->sid[E * lane + r] = sm->ids[x[r] & (N - 1)];
+                __syncwarp();
+            }
+            for (int e = lane; e < m; e += 32) idx[s + e] = sm->sid[e];
+            pk = segment_pairs(sm->sid, s, m, cs, n_s, lane, xi, v, prm);
+            __syncwarp();                                 // ids[], sid[] and slot[] are rewritten by the next segment
+        }
+        packed_sum_ev += pk & 1023; packed_sum_z += (pk >> 10) & 1023; packed_sum_ex += pk >> 20;
+    }
+    const int events = __reduce_add_sync(0xffffffffu, packed_sum_ev);
+    const int zeros = __reduce_add_sync(0xffffffffu, packed_sum_z);
+    const int exact = __reduce_add_sync(0xffffffffu, packed_sum_ex);
+    if (lane == 0) {
+        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+        if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
+    }
+}
+
+// Split cells only: the candidate pair whose members are the last droplet of one segment and the first
+// of the next segment of the same cell.  One thread per segment boundary.
+__global__ void __launch_bounds__(256)
+k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__restrict__ idx,
+                 const int32_t *__restrict__ cell, const int *__restrict__ cell_start,
+                 int64_t *__restrict__ xi, double *__restrict__ v, Ctrl *ctrl,
+                 const __grid_constant__ StepParams prm)
+{
+    const int n = ctrl->n;
+    int events = 0, zeros = 0, exact = 0;
+    for (int seg = blockIdx.x * blockDim.x + threadIdx.x + 1; seg < n_seg; seg += gridDim.x * blockDim.x) {
+        const int p = seg_start[seg];
+        if (p >= n || seg_start[seg - 1] == p) continue;   // an empty predecessor: boundary p belongs to an earlier seg
+        const int a = idx[p - 1], b = idx[p];
+        const int c = cell[a];
+        if (cell[b] != c) continue;
+        const int cs = cell_start[c];
+        if ((p - 1 - cs) & 1) continue;                    // a is a second-in-pair
+        const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
+        const int r = collide_pair_exact(xi, v, a, b, u, pair_norm(cell_start[c + 1] - cs, prm.dtdv), prm.kernel,
+                                         prm.kparam);
+        events += r & 1;
+        zeros += (r >> 1) & 1;
+        exact += 1;
+    }
+    events = __reduce_add_sync(0xffffffffu, events);
+    zeros = __reduce_add_sync(0xffffffffu, zeros);
+    exact = __reduce_add_sync(0xffffffffu, exact);
+    if (lane_id() == 0) {
+        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
+        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
+        if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
     }
 }
 

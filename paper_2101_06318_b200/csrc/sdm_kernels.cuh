@@ -70,11 +70,14 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
     }
 }
 
-__global__ void k_max_count(const int *__restrict__ cell_cnt, int n_cell, Ctrl *ctrl)
+// also clears the counters (invariant of the general path: cell_cnt[] is zero between kernels that use it)
+__global__ void k_max_count(int *__restrict__ cell_cnt, int n_cell, Ctrl *ctrl)
 {
     int m = 0;
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cell; c += gridDim.x * blockDim.x)
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cell; c += gridDim.x * blockDim.x) {
         m = max(m, cell_cnt[c]);
+        cell_cnt[c] = 0;
+    }
     m = __reduce_max_sync(0xffffffffu, m);
     if (lane_id() == 0 && m > 0) atomicMax(&ctrl->max_count, m);
 }
@@ -155,7 +158,7 @@ __device__ __forceinline__ int split_bits(int count, int seg_cap)
 }
 
 __global__ void __launch_bounds__(kScanThreads)
-k_cell_scan(const int *__restrict__ cnt, int n_cell, int *__restrict__ cell_start, int split,
+k_cell_scan(int *__restrict__ cnt, int n_cell, int *__restrict__ cell_start, int split,
             int seg_cap, int *__restrict__ cell_bits, int *__restrict__ bucket_base, Ctrl *ctrl)
 {
     __shared__ int s_warp[33];
@@ -170,21 +173,21 @@ k_cell_scan(const int *__restrict__ cnt, int n_cell, int *__restrict__ cell_star
             loc[k] = (c < n_cell) ? cnt[c] : 0;
             int B = split ? split_bits(loc[k], seg_cap) : 0;
             nb[k] = (c < n_cell) ? (1 << B) : 0;
-            if (split && c < n_cell) cell_bits[c] = B;
+            if (c < n_cell) cell_bits[c] = B;
             sum += loc[k];
             bsum += nb[k];
         }
         int total, btotal = 0;
         int excl = block_exclusive_scan(sum, s_warp, total);
-        int bexcl = 0;
-        if (split) bexcl = block_exclusive_scan(bsum, s_warp, btotal);
+        int bexcl = block_exclusive_scan(bsum, s_warp, btotal);
         int run = carry + excl, brun = bcarry + bexcl;
 #pragma unroll
         for (int k = 0; k < kScanItems; ++k) {
             int c = c0 + k;
             if (c < n_cell) {
                 cell_start[c] = run;
-                if (split) bucket_base[c] = brun;
+                cnt[c] = 0;
+                bucket_base[c] = brun;
             }
             run += loc[k];
             brun += nb[k];
@@ -195,84 +198,13 @@ k_cell_scan(const int *__restrict__ cnt, int n_cell, int *__restrict__ cell_star
     }
     if (threadIdx.x == 0) {
         cell_start[n_cell] = carry;
-        if (split) { bucket_base[n_cell] = bcarry; ctrl->n_buckets = bcarry; }
-    }
-}
-
-// bucket of droplet i: its cell's first bucket + the top B bits of its sort key
-__device__ __forceinline__ int bucket_of(int i, int c, const int *__restrict__ cell_bits,
-                                         const int *__restrict__ bucket_base, uint64_t step,
-                                         const PhiloxKey &rk)
-{
-    int B = cell_bits[c];
-    int b = bucket_base[c];
-    if (B > 0) {
-        uint4 w = droplet_block((uint32_t)i, step, rk);
-        b += (int)(w.y >> (32 - B));
-    }
-    return b;
-}
-
-__global__ void k_bucket_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl,
-                               const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
-                               int *__restrict__ bucket_cnt, uint64_t seed, uint64_t step)
-{
-    PhiloxKey rk;
-    philox_round_keys(seed, rk);
-    const int n = ctrl->n;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-        atomicAdd(&bucket_cnt[bucket_of(i, cell[i], cell_bits, bucket_base, step, rk)], 1);
-}
-
-// exclusive scan of n_buckets counts (n_buckets lives on the device) -> bucket_start[n_buckets+1]
-__global__ void __launch_bounds__(kScanThreads)
-k_bucket_scan(const int *__restrict__ cnt, const Ctrl *__restrict__ ctrl, int *__restrict__ start)
-{
-    __shared__ int s_warp[33];
-    const int nb = ctrl->n_buckets;
-    int carry = 0;
-    for (int base = 0; base < nb; base += kScanThreads * kScanItems) {
-        int c0 = base + threadIdx.x * kScanItems;
-        int loc[kScanItems];
-        int sum = 0;
-#pragma unroll
-        for (int k = 0; k < kScanItems; ++k) {
-            loc[k] = (c0 + k < nb) ? cnt[c0 + k] : 0;
-            sum += loc[k];
-        }
-        int total;
-        int run = carry + block_exclusive_scan(sum, s_warp, total);
-#pragma unroll
-        for (int k = 0; k < kScanItems; ++k) {
-            if (c0 + k < nb) start[c0 + k] = run;
-            run += loc[k];
-        }
-        carry += total;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) start[nb] = carry;
-}
-
-// order[] = droplets grouped by segment (cell, or bucket in split mode); the order inside a
-// segment is arbitrary here -- the segment sort on (key64, storage index) makes it unique.
-__global__ void k_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int split,
-                          const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
-                          const int *__restrict__ seg_start, int *__restrict__ cursor,
-                          int *__restrict__ order, uint64_t seed, uint64_t step)
-{
-    PhiloxKey rk;
-    philox_round_keys(seed, rk);
-    const int n = ctrl->n;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        int c = cell[i];
-        int b = split ? bucket_of(i, c, cell_bits, bucket_base, step, rk) : c;
-        int pos = atomicAdd(&cursor[b], 1);
-        order[seg_start[b] + pos] = i;
+        bucket_base[n_cell] = bcarry;
+        ctrl->n_buckets = bcarry;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Row a3: per-segment sort by (key64, storage index), one warp per segment, in shared memory
+// Row a3 helpers: exact (key64, storage index) order -- bitonic network in shared memory, ranking by counting
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ bool key_less(uint64_t ka, int ia, uint64_t kb, int ib)
 {
@@ -315,82 +247,6 @@ __device__ __noinline__ void warp_rank_by_counting(const int *__restrict__ ids_i
             rank += key_less(key2, id2, key, id) ? 1 : 0;
         }
         idx[out_base + rank] = id;
-    }
-}
-
-// general path: segments described by seg_start[0..n_seg], droplet ids through order[]
-__global__ void __launch_bounds__(kSortWarps * 32)
-k_segment_sort(const int *__restrict__ seg_start, const Ctrl *__restrict__ ctrl, int n_seg_host,
-               int seg_cap, const int *__restrict__ order, int *__restrict__ idx, uint64_t seed,
-               uint64_t step)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = lane_id();
-    uint64_t *skey = reinterpret_cast<uint64_t *>(smem_raw) + warp * kWarpCap;
-    int *sid = reinterpret_cast<int *>(smem_raw + kSortWarps * kWarpCap * sizeof(uint64_t)) + warp * kWarpCap;
-    PhiloxKey rk;
-    philox_round_keys(seed, rk);
-    const int n_seg = n_seg_host >= 0 ? n_seg_host : ctrl->n_buckets;
-    const int warps_total = gridDim.x * kSortWarps;
-    for (int seg = blockIdx.x * kSortWarps + warp; seg < n_seg; seg += warps_total) {
-        const int s = seg_start[seg];
-        const int m = seg_start[seg + 1] - s;
-        if (m == 0) continue;
-        if (m > seg_cap) {
-            warp_rank_by_counting(order + s, 0, m, s, idx, step, rk, lane);
-            continue;
-        }
-        int N = 2;
-        while (N < m) N <<= 1;
-        for (int e = lane; e < N; e += 32) {
-            if (e < m) {
-                int id = order[s + e];
-                skey[e] = block_key64(droplet_block((uint32_t)id, step, rk));
-                sid[e] = id;
-            } else {
-                skey[e] = ~0ull;
-                sid[e] = 0x7fffffff;
-            }
-        }
-        __syncwarp();
-        warp_bitonic(skey, sid, N, lane);
-        for (int e = lane; e < m; e += 32) idx[s + e] = sid[e];
-        __syncwarp();
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Rows a4-a6 (general path): pairs by position in idx, as Fig. 4 flags them
-// ---------------------------------------------------------------------------------------------
-__global__ void k_pairs_by_position(int64_t *__restrict__ xi, double *__restrict__ v,
-                                    const int32_t *__restrict__ cell, const int *__restrict__ idx,
-                                    const int *__restrict__ cell_start, Ctrl *ctrl, StepParams prm)
-{
-    PhiloxKey rk;
-    philox_round_keys(prm.seed, rk);
-    const int n = ctrl->n;
-    int events = 0, zeros = 0, exact = 0;
-    for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
-        int a = idx[p];
-        int c = cell[a];
-        int s = cell_start[c];
-        int n_s = cell_start[c + 1] - s;
-        bool first = (((p - s) & 1) == 0) && (p + 1 < s + n_s);     // Fig. 4
-        if (!first) continue;
-        int b = idx[p + 1];
-        double u = block_uniform(droplet_block((uint32_t)a, prm.step, rk));
-        int r = collide_pair_exact(xi, v, a, b, u, pair_norm(n_s, prm.dtdv), prm.kernel, prm.kparam);
-        events += r & 1;
-        zeros += (r >> 1) & 1;
-        exact += 1;
-    }
-    events = __reduce_add_sync(0xffffffffu, events);
-    zeros = __reduce_add_sync(0xffffffffu, zeros);
-    exact = __reduce_add_sync(0xffffffffu, exact);
-    if (lane_id() == 0) {
-        if (events) atomicAdd(&ctrl->n_events, (unsigned long long)events);
-        if (zeros) atomicAdd(&ctrl->zero_count, zeros);
-        if (exact) atomicAdd(&ctrl->n_exact, (unsigned long long)exact);
     }
 }
 
