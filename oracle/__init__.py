@@ -48,6 +48,13 @@ def lib() -> C.CDLL:
         L.orc_step.restype = C.c_int
         L.orc_remove_zero.argtypes = [C.c_int64, p, p, p]
         L.orc_remove_zero.restype = C.c_int64
+        L.orc_collide_pair_attr.argtypes = [p, p, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int64]
+        L.orc_collide_pair_attr.restype = None
+        L.orc_step_attr.argtypes = [C.c_int64, p, p, C.c_int32, C.c_int64, p, C.c_int32, p, C.c_double, C.c_double,
+                                    C.c_int32, C.c_double, C.c_uint64, C.c_uint64, p, p, p]
+        L.orc_step_attr.restype = C.c_int
+        L.orc_remove_zero_attr.argtypes = [C.c_int64, p, p, C.c_int32, C.c_int64, p]
+        L.orc_remove_zero_attr.restype = C.c_int64
         L.orc_moments.argtypes = [C.c_int64, p, p, p, C.c_int32, C.c_int32, p, p, p]
         L.orc_moments.restype = None
     return _lib
@@ -140,6 +147,43 @@ def step(xi, v, cell_id, n_cell, dt, dV, ktype, kparam, seed, step, sid=None, wa
     if rc != 0:
         raise ValueError("orc_step: invalid input")
     return idx, cs, nev.value
+
+
+def collide_pair_attr(xi, attr, a, b, gamma):
+    """Fig. 5 body IN PLACE on xi[n] and the row-major attribute block attr[n_attr, n] (row 0 = volume)
+    for the pair (a = first-in-pair, b) with uncapped gamma."""
+    xi = _chk(xi, np.int64)
+    attr = _chk(attr, np.float64)
+    assert attr.ndim == 2 and attr.shape[1] == xi.shape[0]
+    lib().orc_collide_pair_attr(_ptr(xi), _ptr(attr), attr.shape[0], attr.shape[1], int(a), int(b), int(gamma))
+
+
+def step_attr(xi, attr, cell_id, n_cell, dt, dV, ktype, kparam, seed, step, want_perm=True):
+    """One coalescence step IN PLACE on xi[n] and attr[n_attr, n] (row 0 = volume).
+    Returns (idx, cell_start, n_events)."""
+    xi = _chk(xi, np.int64)
+    attr = _chk(attr, np.float64)
+    cell_id = _chk(cell_id, np.int32)
+    n = xi.shape[0]
+    assert attr.ndim == 2 and attr.shape[1] == n and cell_id.shape[0] == n
+    idx = np.empty(n, dtype=np.int32) if want_perm else None
+    cs = np.empty(n_cell + 1, dtype=np.int32) if want_perm else None
+    nev = C.c_int64(0)
+    rc = lib().orc_step_attr(n, _ptr(xi), _ptr(attr), attr.shape[0], n, _ptr(cell_id), n_cell, None, float(dt),
+                             float(dV), int(ktype), float(kparam), int(seed), int(step), _ptr(idx), _ptr(cs),
+                             C.byref(nev))
+    if rc != 0:
+        raise ValueError("orc_step_attr: invalid input")
+    return idx, cs, nev.value
+
+
+def remove_zero_attr(xi, attr, cell_id):
+    """Stable removal of xi == 0 with all attribute rows.  Returns trimmed COPIES (xi, attr, cell_id)."""
+    xi = _chk(xi, np.int64).copy()
+    attr = _chk(attr, np.float64).copy()
+    cell_id = _chk(cell_id, np.int32).copy()
+    m = lib().orc_remove_zero_attr(xi.shape[0], _ptr(xi), _ptr(attr), attr.shape[0], attr.shape[1], _ptr(cell_id))
+    return xi[:m].copy(), np.ascontiguousarray(attr[:, :m]), cell_id[:m].copy()
 
 
 def remove_zero(xi, v, cell_id):

@@ -192,38 +192,56 @@ int64_t orc_gamma_tilde(double p, double u, int64_t xi_j, int64_t xi_k)
     return g < q ? g : q;
 }
 
-/* Fig. 5 for one pair, one attribute. */
-void orc_collide_pair(int64_t *xi_a, double *v_a, int64_t *xi_b, double *v_b, int64_t gamma)
+/* Fig. 5 for one pair (a = first-in-pair, b = second) and n_attr extensive
+ * attributes stored as rows of a 2-D row-major array with leading dimension ld (PAPER.md:138, 145:
+ * "attributes = Storage((N_ATTR, N_SD), float)"; the loop "for attr in range(len(attributes))" at
+ * PAPER.md:271-287).  Row 0 is the volume (volume_view). */
+void orc_collide_pair_attr(int64_t *xi, double *attr, int32_t n_attr, int64_t ld, int64_t a, int64_t b,
+                           int64_t gamma)
 {
-    int64_t *nj = xi_a, *nk = xi_b;
-    double *aj = v_a, *ak = v_b;
-    if (*nj < *nk) {
-        nj = xi_b; nk = xi_a; aj = v_b; ak = v_a;
-    }
-    if (*nk == 0) return;                             /* DESIGN.md R11: zero-xi partner */
-    int64_t q = *nj / *nk;
+    int64_t j = a, k = b;
+    if (xi[j] < xi[k]) { j = b; k = a; }
+    if (xi[k] == 0) return;                           /* DESIGN.md R11: zero-xi partner */
+    int64_t q = xi[j] / xi[k];
     int64_t g = gamma < q ? gamma : q;                /* PAPER.md:260 (Eq. 4) */
     if (g == 0) return;
-    int64_t new_n = *nj - g * *nk;
+    int64_t new_n = xi[j] - g * xi[k];
     if (new_n > 0) {                                  /* Eq. 5 */
-        *nj = new_n;
-        double t = (double)g * *aj;
-        *ak = *ak + t;
+        xi[j] = new_n;
+        for (int32_t r = 0; r < n_attr; ++r) {
+            double *A = attr + (int64_t)r * ld;
+            double t = (double)g * A[j];
+            A[k] = A[k] + t;
+        }
     } else {                                          /* Eq. 6 */
-        *nj = *nk / 2;
-        *nk = *nk - *nj;
-        double t = *aj * (double)g;
-        *aj = t + *ak;
-        *ak = *aj;
+        xi[j] = xi[k] / 2;
+        xi[k] = xi[k] - xi[j];
+        for (int32_t r = 0; r < n_attr; ++r) {
+            double *A = attr + (int64_t)r * ld;
+            double t = A[j] * (double)g;
+            A[j] = t + A[k];
+            A[k] = A[j];
+        }
     }
 }
 
-int orc_step(int64_t n, int64_t *xi, double *v, const int32_t *cell_id, int32_t n_cell,
-             const int64_t *sid, double dt, double dV, int32_t kernel, double kparam,
-             uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
-             int64_t *n_events_out)
+/* One pair, one attribute, operands by pointer (the form the pair-level pins use). */
+void orc_collide_pair(int64_t *xi_a, double *v_a, int64_t *xi_b, double *v_b, int64_t gamma)
 {
-    if (n < 0 || n_cell < 1) return -1;
+    int64_t xi[2] = { *xi_a, *xi_b };
+    double A[2] = { *v_a, *v_b };
+    orc_collide_pair_attr(xi, A, 1, 2, 0, 1, gamma);
+    *xi_a = xi[0]; *xi_b = xi[1]; *v_a = A[0]; *v_b = A[1];
+}
+
+int orc_step_attr(int64_t n, int64_t *xi, double *attr, int32_t n_attr, int64_t ld,
+                  const int32_t *cell_id, int32_t n_cell,
+                  const int64_t *sid, double dt, double dV, int32_t kernel, double kparam,
+                  uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
+                  int64_t *n_events_out)
+{
+    if (n < 0 || n_cell < 1 || n_attr < 1 || ld < n) return -1;
+    double *v = attr;                                 /* volume_view = attributes[0, :] */
     uint64_t *key64 = (uint64_t *)malloc((size_t)(n + 1) * sizeof(uint64_t));
     double *ucand = (double *)malloc((size_t)(n + 1) * sizeof(double));
     int32_t *idx = (int32_t *)malloc((size_t)(n + 1) * sizeof(int32_t));
@@ -253,7 +271,7 @@ int orc_step(int64_t n, int64_t *xi, double *v, const int32_t *cell_id, int32_t 
             if (g == 0) continue;
             n_events += 1;
             /* gamma_tilde <= floor(xi_j/xi_k), so passing it as gamma leaves it unchanged */
-            orc_collide_pair(&xi[a], &v[a], &xi[b], &v[b], g);
+            orc_collide_pair_attr(xi, attr, n_attr, ld, a, b, g);
         }
     }
     if (idx_out) memcpy(idx_out, idx, (size_t)n * sizeof(int32_t));
@@ -264,17 +282,34 @@ done:
     return rc;
 }
 
-/* Step 0: filter, order preserved (R12). */
-int64_t orc_remove_zero(int64_t n, int64_t *xi, double *v, int32_t *cell_id)
+int orc_step(int64_t n, int64_t *xi, double *v, const int32_t *cell_id, int32_t n_cell,
+             const int64_t *sid, double dt, double dV, int32_t kernel, double kparam,
+             uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
+             int64_t *n_events_out)
+{
+    return orc_step_attr(n, xi, v, 1, n, cell_id, n_cell, sid, dt, dV, kernel, kparam, seed, step,
+                         idx_out, cell_start_out, n_events_out);
+}
+
+/* Step 0: filter, order preserved (R12); every attribute row moves
+ * with its droplet. */
+int64_t orc_remove_zero_attr(int64_t n, int64_t *xi, double *attr, int32_t n_attr, int64_t ld,
+                             int32_t *cell_id)
 {
     int64_t m = 0;
     for (int64_t i = 0; i < n; ++i) {
         if (xi[i] != 0) {
-            xi[m] = xi[i]; v[m] = v[i]; cell_id[m] = cell_id[i];
+            xi[m] = xi[i]; cell_id[m] = cell_id[i];
+            for (int32_t r = 0; r < n_attr; ++r) attr[(int64_t)r * ld + m] = attr[(int64_t)r * ld + i];
             m += 1;
         }
     }
     return m;
+}
+
+int64_t orc_remove_zero(int64_t n, int64_t *xi, double *v, int32_t *cell_id)
+{
+    return orc_remove_zero_attr(n, xi, v, 1, n, cell_id);
 }
 
 /* Neumaier compensated accumulation: sum += x with a running error term. */

@@ -61,6 +61,11 @@ int64_t orc_gamma_tilde(double p, double u, int64_t xi_j, int64_t xi_k);
  * extensive attribute, given the UNCAPPED gamma.  (a, b) is (first-in-pair, second). */
 void orc_collide_pair(int64_t *xi_a, double *v_a, int64_t *xi_b, double *v_b, int64_t gamma);
 
+/* The same for n_attr extensive attributes, rows of a row-major (n_attr, ld) array, row 0 = volume
+ * (PAPER.md:138, 145-147, 271-287); a, b index the droplets (a = first-in-pair). */
+void orc_collide_pair_attr(int64_t *xi, double *attr, int32_t n_attr, int64_t ld, int64_t a, int64_t b,
+                           int64_t gamma);
+
 /* One coalescence step (Fig. 3 steps 1-3) in place on (xi, v).
  * idx_out[n], cell_start_out[n_cell+1] may be NULL.  sid may be NULL (identity).
  * n_events_out (may be NULL): number of pairs with gamma_tilde > 0.
@@ -70,7 +75,16 @@ int orc_step(int64_t n, int64_t *xi, double *v, const int32_t *cell_id, int32_t 
              uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
              int64_t *n_events_out);
 
+/* orc_step with n_attr >= 1 extensive attributes (row 0 = volume, which alone enters Eq. 3). */
+int orc_step_attr(int64_t n, int64_t *xi, double *attr, int32_t n_attr, int64_t ld,
+                  const int32_t *cell_id, int32_t n_cell,
+                  const int64_t *sid, double dt, double dV, int32_t kernel, double kparam,
+                  uint64_t seed, uint64_t step, int32_t *idx_out, int32_t *cell_start_out,
+                  int64_t *n_events_out);
+
 /* Step 0: drop xi == 0, keep storage order.  Returns survivors. */
+int64_t orc_remove_zero_attr(int64_t n, int64_t *xi, double *attr, int32_t n_attr, int64_t ld,
+                             int32_t *cell_id);
 int64_t orc_remove_zero(int64_t n, int64_t *xi, double *v, int32_t *cell_id);
 
 /* Moments M_k = sum xi v^k, k = 0,1,2 (R13).  per_cell == 0:
