@@ -75,12 +75,23 @@ enum {
  * arguments are invalid (capacity < 1, capacity >= 2^31 - 1024, n_cell < 1). */
 size_t sdm_workspace_bytes(int64_t capacity, int32_t n_cell);
 
+/* The same for a state with n_attr extensive attributes per super-droplet (1 <= n_attr <= SDM_MAX_ATTR):
+ * the paper's `attributes = Storage((N_ATTR, N_SD), float)`, a 2-D row-major block whose row 0 is the
+ * volume (`volume_view`).  n_attr == 1 equals sdm_workspace_bytes. */
+#define SDM_MAX_ATTR 8
+size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr);
+
 /* Creates a handle.  workspace_dev: caller-owned device memory, 256-byte aligned, at least
  * sdm_workspace_bytes(capacity, n_cell) bytes.  cuda_stream: a cudaStream_t (NULL = legacy default
  * stream).  The state is empty (n_sd = 0) until sdm_set_state.  Synchronous (clears the control
  * block).  Errors: SDM_EINVAL (bad arguments, workspace too small or misaligned), SDM_ECUDA. */
 int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_dev,
                size_t workspace_bytes, void *cuda_stream);
+
+/* sdm_create for n_attr extensive attributes (sdm_create is n_attr = 1); the workspace must hold
+ * sdm_workspace_bytes_attr(capacity, n_cell, n_attr) bytes. */
+int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_attr, void *workspace_dev,
+                    size_t workspace_bytes, void *cuda_stream);
 
 /* Frees the handle (host memory only; the workspace stays with the caller).  Synchronises the stream. */
 int sdm_destroy(sdm_t *h);
@@ -95,6 +106,18 @@ int sdm_set_state(sdm_t *h, int64_t n_sd, const int64_t *xi_dev, const double *v
                   const int32_t *cell_id_dev);
 int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const double *v_host,
                        const int32_t *cell_id_host);
+
+/* Rows 1 .. n_attr-1 of the attribute block (row 0, the volume, goes through sdm_set_state): row r is read
+ * from attr_dev + (r-1)*ld, n_sd values each, ld >= n_sd in elements.  Call it after sdm_set_state, which
+ * zero-fills these rows; n_sd is that call's n_sd.  Every value must be finite (else SDM_EINVAL and the
+ * state becomes unusable).  The rows are updated by every coalescence event exactly like the volume
+ * (Fig. 5 loop over attributes: A_k += g A_j, or both g A_j + A_k on the split branch),
+ * move with their droplet in sdm_remove_zero, and never enter Eq. 3.  SYNCHRONOUS.  SDM_EINVAL if the
+ * handle has n_attr == 1. */
+int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld);
+
+/* Copies rows 1 .. n_attr-1 out (row r to attr_dev + (r-1)*ld, current n_sd values each).  SYNCHRONOUS. */
+int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld);
 
 /* Copies the current state out in storage order.  Any of the array pointers may be NULL.
  * SYNCHRONOUS (returns n_sd on the host).  The arrays must hold at least n_sd elements (capacity

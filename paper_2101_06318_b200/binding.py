@@ -32,7 +32,9 @@ SYMBOLS = (
     "sdm_set_state", "sdm_set_state_host", "sdm_get_state", "sdm_get_state_host",
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
+    "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
 )
+MAX_ATTR = 8
 
 
 class SdmError(RuntimeError):
@@ -68,6 +70,11 @@ def load_library() -> C.CDLL:
     L.sdm_workspace_bytes.argtypes = [i64, i32]
     L.sdm_workspace_bytes.restype = C.c_size_t
     L.sdm_create.argtypes = [C.POINTER(vp), i64, i32, vp, C.c_size_t, vp]
+    L.sdm_workspace_bytes_attr.argtypes = [i64, i32, i32]
+    L.sdm_workspace_bytes_attr.restype = C.c_size_t
+    L.sdm_create_attr.argtypes = [C.POINTER(vp), i64, i32, i32, vp, C.c_size_t, vp]
+    L.sdm_set_attributes.argtypes = [vp, vp, i64]
+    L.sdm_get_attributes.argtypes = [vp, vp, i64]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
     L.sdm_set_state.argtypes = [vp, i64, vp, vp, vp]
@@ -86,7 +93,7 @@ def load_library() -> C.CDLL:
     L.sdm_last_error.argtypes = [vp]
     L.sdm_last_error.restype = C.c_char_p
     for name in SYMBOLS:
-        if name not in ("sdm_workspace_bytes", "sdm_last_error"):
+        if name not in ("sdm_workspace_bytes", "sdm_workspace_bytes_attr", "sdm_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -96,8 +103,8 @@ def version() -> int:
     return load_library().sdm_version()
 
 
-def workspace_bytes(capacity: int, n_cell: int) -> int:
-    return int(load_library().sdm_workspace_bytes(capacity, n_cell))
+def workspace_bytes(capacity: int, n_cell: int, n_attr: int = 1) -> int:
+    return int(load_library().sdm_workspace_bytes_attr(capacity, n_cell, n_attr))
 
 
 def _kernel(kernel: int, kparam: float) -> KernelDesc:
@@ -110,7 +117,7 @@ class SDM:
     """One simulation state on one GPU.  Device memory (workspace) is a torch tensor; the stream is
     torch's current stream at construction."""
 
-    def __init__(self, capacity: int, n_cell: int, device="cuda:0", stream=None):
+    def __init__(self, capacity: int, n_cell: int, device="cuda:0", stream=None, n_attr: int = 1):
         import torch
 
         self._lib = load_library()
@@ -118,18 +125,18 @@ class SDM:
             raise RuntimeError("no CUDA device: libsdm has no CPU fallback")
         self.torch = torch
         self.device = torch.device(device)
-        self.capacity, self.n_cell = int(capacity), int(n_cell)
-        nbytes = workspace_bytes(self.capacity, self.n_cell)
+        self.capacity, self.n_cell, self.n_attr = int(capacity), int(n_cell), int(n_attr)
+        nbytes = workspace_bytes(self.capacity, self.n_cell, self.n_attr)
         if nbytes == 0:
-            raise SdmError(SDM_EINVAL, "invalid capacity / n_cell")
+            raise SdmError(SDM_EINVAL, "invalid capacity / n_cell / n_attr")
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = self.workspace.data_ptr()
             self._ws_ptr = (base + 255) // 256 * 256
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
-            rc = self._lib.sdm_create(C.byref(h), self.capacity, self.n_cell, C.c_void_p(self._ws_ptr),
-                                      nbytes, C.c_void_p(self.stream.cuda_stream))
+            rc = self._lib.sdm_create_attr(C.byref(h), self.capacity, self.n_cell, self.n_attr,
+                                           C.c_void_p(self._ws_ptr), nbytes, C.c_void_p(self.stream.cuda_stream))
         if rc != SDM_OK:
             raise SdmError(rc, self._lib.sdm_last_error(None).decode())
         self._h = h
@@ -179,6 +186,20 @@ class SDM:
         n = xi.shape[0]
         self._host(xi, t.int64), self._host(v, t.float64), self._host(cell_id, t.int32)
         self._check(self._lib.sdm_set_state_host(self._h, n, self._p(xi), self._p(v), self._p(cell_id)))
+
+    def set_attributes(self, attr):
+        """Rows 1..n_attr-1 of the attribute block: a contiguous float64 device tensor [n_attr-1, n_sd]."""
+        self._dev(attr, self.torch.float64)
+        assert attr.dim() == 2 and attr.shape[0] == self.n_attr - 1
+        self._check(self._lib.sdm_set_attributes(self._h, self._p(attr), int(attr.shape[1])))
+
+    def get_attributes(self):
+        """Returns rows 1..n_attr-1 as a device tensor [n_attr-1, n_sd] (current n_sd)."""
+        t = self.torch
+        n = self.counters()["n_sd"]
+        out = t.empty((self.n_attr - 1, max(n, 1)), dtype=t.float64, device=self.device)
+        self._check(self._lib.sdm_get_attributes(self._h, self._p(out), int(out.shape[1])))
+        return out[:, :n]
 
     def get_state(self):
         """Returns (xi, v, cell_id) device tensors trimmed to the current n_sd."""

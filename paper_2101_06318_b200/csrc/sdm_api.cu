@@ -28,12 +28,12 @@ constexpr int kMinSegCap = 8;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t xi, v, cell, idx, order, cell_start, cell_cnt, cell_bits, bucket_base, bucket_start,
+    size_t xi, v, attr, cell, idx, order, cell_start, cell_cnt, cell_bits, bucket_base, bucket_start,
         bucket_cnt, tile_status, part0, part1, part2, mom_out, ctrl, total;
-    int64_t nb_max, n_tiles;
+    int64_t nb_max, n_tiles, attr_stride;
 };
 
-Layout make_layout(int64_t cap, int32_t n_cell)
+Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
 {
     Layout L{};
     L.nb_max = (int64_t)n_cell + cap / 64 + 4096;
@@ -42,6 +42,8 @@ Layout make_layout(int64_t cap, int32_t n_cell)
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     L.xi = take((size_t)cap * 8);
     L.v = take((size_t)cap * 8);
+    L.attr_stride = (cap + 31) / 32 * 32;                       // elements between rows of the extra attributes
+    L.attr = take((size_t)(n_attr - 1) * (size_t)L.attr_stride * 8);
     L.cell = take((size_t)cap * 4);
     L.idx = take((size_t)cap * 4);
     L.order = take((size_t)cap * 4);
@@ -68,6 +70,8 @@ thread_local std::string g_create_error;
 struct sdm {
     int64_t capacity = 0;
     int32_t n_cell = 0;
+    int32_t n_attr = 1;          // extensive attributes per droplet, volume included
+    double *attr = nullptr;      // rows 1..n_attr-1
     cudaStream_t stream = nullptr;
     unsigned char *ws = nullptr;
     Layout L{};
@@ -181,6 +185,15 @@ bool use_fused(const sdm_t *h)
 int general_cap(const sdm_t *h) { return h->seg_cap_set ? h->seg_cap : kGenCap; }
 
 
+AttrView attr_view(const sdm_t *h)
+{
+    AttrView av{};
+    av.p = h->attr;
+    av.stride = h->L.attr_stride;
+    av.n = h->n_attr - 1;
+    return av;
+}
+
 int read_ctrl(sdm_t *h)
 {
     SDM_CUDA(h, cudaMemcpyAsync(h->ctrl_host, h->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->stream));
@@ -208,6 +221,7 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.step = step;
     prm.screening = h->screening ? 1 : 0;
     prm.sort_fallback = h->sort_fallback ? 1 : 0;
+    prm.attr = attr_view(h);
     philox_round_keys(seed, prm.rk);
     return SDM_OK;
 }
@@ -312,8 +326,8 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
 int enqueue_remove_zero(sdm_t *h)
 {
     int64_t tiles = (h->n_ub + kCompactTile - 1) / kCompactTile;
-    SDM_LAUNCH(h, k_compact, grid_for(h, tiles * kCompactThreads, kCompactThreads, 4), kCompactThreads, 0,
-               h->xi, h->v, h->cell, h->ctrl, h->tile_status);
+    SDM_LAUNCH(h, k_compact, grid_for(h, tiles * kCompactThreads, kCompactThreads, 4), kCompactThreads,
+               (size_t)(h->n_attr - 1) * kCompactTile * 8, h->xi, h->v, h->cell, h->ctrl, h->tile_status, attr_view(h));
     h->stepped = false;                       // idx no longer refers to the current storage order
     return SDM_OK;
 }
@@ -338,6 +352,8 @@ int load_state_common(sdm_t *h, int64_t n_sd)
     zero.n = (int)n_sd;
     zero.epoch = 1;                                   // tile status words are tagged; 0 = never written
     SDM_CUDA(h, cudaMemsetAsync(h->tile_status, 0, (size_t)h->L.n_tiles * 8, h->stream));
+    if (h->n_attr > 1)
+        SDM_CUDA(h, cudaMemsetAsync(h->attr, 0, (size_t)(h->n_attr - 1) * (size_t)h->L.attr_stride * 8, h->stream));
     SDM_CUDA(h, cudaMemcpyAsync(h->ctrl, &zero, sizeof(Ctrl), cudaMemcpyHostToDevice, h->stream));
     SDM_CUDA(h, cudaStreamSynchronize(h->stream));   // `zero` lives on this stack frame
     SDM_CUDA(h, cudaMemsetAsync(h->cell_cnt, 0, ((size_t)h->n_cell + 1) * 4, h->stream));
@@ -365,23 +381,32 @@ int load_state_common(sdm_t *h, int64_t n_sd)
 
 extern "C" {
 
-int sdm_version(void) { return 1000; }
+int sdm_version(void) { return 1001; }
 
-size_t sdm_workspace_bytes(int64_t capacity, int32_t n_cell)
+size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
-    if (capacity < 1 || capacity >= (int64_t)0x7fffffff - 1024 || n_cell < 1) return 0;
-    return make_layout(capacity, n_cell).total;
+    if (capacity < 1 || capacity >= (int64_t)0x7fffffff - 1024 || n_cell < 1 || n_attr < 1 || n_attr > SDM_MAX_ATTR)
+        return 0;
+    return make_layout(capacity, n_cell, n_attr).total;
 }
+
+size_t sdm_workspace_bytes(int64_t capacity, int32_t n_cell) { return sdm_workspace_bytes_attr(capacity, n_cell, 1); }
 
 const char *sdm_last_error(const sdm_t *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_dev, size_t workspace_bytes,
                void *cuda_stream)
 {
+    return sdm_create_attr(out, capacity, n_cell, 1, workspace_dev, workspace_bytes, cuda_stream);
+}
+
+int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_attr, void *workspace_dev,
+                    size_t workspace_bytes, void *cuda_stream)
+{
     if (!out) return fail(nullptr, SDM_EINVAL, "out is NULL");
     *out = nullptr;
-    size_t need = sdm_workspace_bytes(capacity, n_cell);
-    if (need == 0) return fail(nullptr, SDM_EINVAL, "invalid capacity or n_cell");
+    size_t need = sdm_workspace_bytes_attr(capacity, n_cell, n_attr);
+    if (need == 0) return fail(nullptr, SDM_EINVAL, "invalid capacity, n_cell or n_attr");
     if (!workspace_dev) return fail(nullptr, SDM_EINVAL, "workspace is NULL");
     if (reinterpret_cast<uintptr_t>(workspace_dev) % kAlign != 0)
         return fail(nullptr, SDM_EINVAL, "workspace must be 256-byte aligned");
@@ -398,11 +423,13 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     h->n_cell = n_cell;
     h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     h->ws = static_cast<unsigned char *>(workspace_dev);
-    h->L = make_layout(capacity, n_cell);
+    h->n_attr = n_attr;
+    h->L = make_layout(capacity, n_cell, n_attr);
     h->num_sms = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     const Layout &L = h->L;
     h->xi = reinterpret_cast<int64_t *>(h->ws + L.xi);
     h->v = reinterpret_cast<double *>(h->ws + L.v);
+    h->attr = reinterpret_cast<double *>(h->ws + L.attr);
     h->cell = reinterpret_cast<int32_t *>(h->ws + L.cell);
     h->idx = reinterpret_cast<int *>(h->ws + L.idx);
     h->order = reinterpret_cast<int *>(h->ws + L.order);
@@ -434,6 +461,11 @@ int sdm_create(sdm_t **out, int64_t capacity, int32_t n_cell, void *workspace_de
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<true>)");
     e = cudaFuncSetAttribute(k_fused_cells_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<false>)");
+    if (n_attr > 1) {
+        e = cudaFuncSetAttribute(k_compact, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)((SDM_MAX_ATTR - 1) * kCompactTile * 8));
+        if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_compact)");
+    }
     e = cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(ctrl)");
     e = cudaMemsetAsync(h->cell_cnt, 0, ((size_t)n_cell + 1) * 4, h->stream);
@@ -521,6 +553,46 @@ int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const dou
         SDM_CUDA(h, cudaMemcpyAsync(h->cell, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, h->stream));
     }
     return load_state_common(h, n_sd);
+}
+
+int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld)
+{
+    if (!h) return SDM_EINVAL;
+    if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
+    if (h->n_attr < 2) return fail(h, SDM_EINVAL, "the handle was created with n_attr = 1");
+    int rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    const int64_t n = h->ctrl_host->n;
+    h->n_ub = n;
+    if (n == 0) return SDM_OK;
+    if (!attr_dev || ld < n) return fail(h, SDM_EINVAL, "attribute pointer is NULL or ld < n_sd");
+    SDM_CUDA(h, cudaMemcpy2DAsync(h->attr, (size_t)h->L.attr_stride * 8, attr_dev, (size_t)ld * 8, (size_t)n * 8,
+                                  (size_t)(h->n_attr - 1), cudaMemcpyDeviceToDevice, h->stream));
+    SDM_LAUNCH(h, k_check_attr, grid_for(h, n, 256, 8), 256, 0, attr_view(h), (int)n, h->ctrl);
+    rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    if (h->ctrl_host->invalid) {
+        h->valid = false;
+        return fail(h, SDM_EINVAL, "attribute validation failed: every value must be finite");
+    }
+    return SDM_OK;
+}
+
+int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld)
+{
+    if (!h) return SDM_EINVAL;
+    if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
+    if (h->n_attr < 2) return fail(h, SDM_EINVAL, "the handle was created with n_attr = 1");
+    int rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    const int64_t n = h->ctrl_host->n;
+    h->n_ub = n;
+    if (n == 0) return SDM_OK;
+    if (!attr_dev || ld < n) return fail(h, SDM_EINVAL, "attribute pointer is NULL or ld < n_sd");
+    SDM_CUDA(h, cudaMemcpy2DAsync(attr_dev, (size_t)ld * 8, h->attr, (size_t)h->L.attr_stride * 8, (size_t)n * 8,
+                                  (size_t)(h->n_attr - 1), cudaMemcpyDeviceToDevice, h->stream));
+    SDM_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SDM_OK;
 }
 
 static int get_state_impl(sdm_t *h, int64_t *n_sd, int64_t *xi, double *v, int32_t *cell, cudaMemcpyKind kind)

@@ -65,6 +65,16 @@ __device__ __forceinline__ double block_uniform(const uint4 &w)
 // ---------------------------------------------------------------------------------------------
 // Row a5: coalescence kernels (R9, R10) and Eq. 3.
 // ---------------------------------------------------------------------------------------------
+// Extensive attributes other than the volume: rows 1..N_ATTR-1
+// of the paper's 2-D row-major attribute block, row r at p + r*stride.  They never enter Eq. 3; only a pair
+// with gamma_tilde > 0 touches them.
+struct AttrView {
+    double *p;
+    long long stride;
+    int n;                  // number of extra rows (0: volume is the only attribute)
+    int pad;
+};
+
 struct StepParams {
     double dtdv;      // dt / dV, one IEEE division on the host
     double kparam;    // Golovin b, or gravitational E
@@ -73,6 +83,7 @@ struct StepParams {
     uint64_t seed, step;
     int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
     int32_t sort_fallback;  // unused (kept for ABI stability of the option numbering)
+    AttrView attr;          // extra extensive attributes
     PhiloxKey rk;           // round keys of `seed`: kernels that take the parameters as __grid_constant__ read
                             // them straight from the constant bank instead of holding 20 registers
 };
@@ -133,7 +144,7 @@ __device__ __forceinline__ double pair_norm(int n_s, double dtdv)
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, double *__restrict__ v,
                                                   int a, int b, double u, double norm,
-                                                  int32_t ktype, double kparam)
+                                                  int32_t ktype, double kparam, const AttrView &av)
 {
     int64_t xa = xi[a], xb = xi[b];
     int j = a, k = b;
@@ -155,11 +166,16 @@ __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, doub
     }
     if (g == 0) return 0;
     int64_t new_n = xj - g * xk;
-    double gv = __dmul_rn(__ll2double_rn(g), vj);
+    const double gd = __ll2double_rn(g);
+    double gv = __dmul_rn(gd, vj);
     double vnew = __dadd_rn(vk, gv);                     // both branches produce v_k + g v_j
     if (new_n > 0) {                                     // Eq. 5
         xi[j] = new_n;
         v[k] = vnew;
+        for (int r = 0; r < av.n; ++r) {                 // every extensive attribute
+            double *A = av.p + (long long)r * av.stride;
+            A[k] = __dadd_rn(A[k], __dmul_rn(gd, A[j]));
+        }
         return 1;
     }
     int64_t half = xk >> 1;                              // Eq. 6, xk > 0
@@ -167,6 +183,12 @@ __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, doub
     xi[k] = xk - half;
     v[j] = vnew;
     v[k] = vnew;
+    for (int r = 0; r < av.n; ++r) {
+        double *A = av.p + (long long)r * av.stride;
+        const double t = __dadd_rn(A[k], __dmul_rn(gd, A[j]));
+        A[j] = t;
+        A[k] = t;
+    }
     return half == 0 ? 3 : 1;
 }
 

@@ -166,7 +166,7 @@ __device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v,
 __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int L, int lane0,
                                             int64_t *xi, double *v, int s, int n_s, int li, double dtdv,
                                             int32_t ktype, double kparam, uint64_t seed, uint64_t step,
-                                            double *delta)
+                                            double *delta, const AttrView &av)
 {
     const uint32_t N = (uint32_t)(E * L);
     int64_t d0 = 0;
@@ -185,7 +185,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
         int64_t o0 = 0;
         double o1 = 0.0, o2 = 0.0;
         if (delta) pair_moments(xi, v, s + a, s + b, o0, o1, o2);
-        const int r = collide_pair_exact(xi, v, s + a, s + b, u, norm, ktype, kparam);
+        const int r = collide_pair_exact(xi, v, s + a, s + b, u, norm, ktype, kparam, av);
         if (delta && (r & 1)) {
             int64_t n0;
             double n1, n2;
@@ -208,7 +208,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 // sdm_set_state and cells never grow); this keeps the result defined anyway.  Whole warp, one cell.
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
                                           double dtdv, int32_t ktype, double kparam, uint64_t seed,
-                                          uint64_t step, double *delta)
+                                          uint64_t step, double *delta, const AttrView &av)
 {
     PhiloxKey rk;
     philox_round_keys(seed, rk);
@@ -219,7 +219,7 @@ __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int 
     for (int q = lane; q < (n_s >> 1); q += 32) {
         int a = idx[s + 2 * q], b = idx[s + 2 * q + 1];
         double u = block_uniform(droplet_block((uint32_t)a, step, rk));
-        int r = collide_pair_exact(xi, v, a, b, u, norm, ktype, kparam);
+        int r = collide_pair_exact(xi, v, a, b, u, norm, ktype, kparam, av);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
     if (delta) {                                      // here: the cell's whole post-step contribution
@@ -282,7 +282,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
                 const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
                 if (n2 <= N) continue;
                 const int pk = oversize_cell(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
-                                             prm.seed, prm.step, my_delta);
+                                             prm.seed, prm.step, my_delta, prm.attr);
                 events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
                 if (MOM) {
                     a0 += __double_as_longlong(my_delta[0]);
@@ -396,7 +396,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
             __syncwarp();
             const int pk = collide_flagged(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
-                                           prm.kernel, prm.kparam, prm.seed, prm.step, my_delta);
+                                           prm.kernel, prm.kparam, prm.seed, prm.step, my_delta, prm.attr);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
             if (MOM) {
                 a0 += __double_as_longlong(my_delta[0]);

@@ -70,6 +70,18 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
     }
 }
 
+// sdm_set_attributes: every value of the extra attribute rows must be finite
+__global__ void k_check_attr(const AttrView av, int n, Ctrl *ctrl)
+{
+    int bad = 0;
+    for (int r = 0; r < av.n; ++r)
+        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+            const double a = av.p[(long long)r * av.stride + i];
+            if (!(fabs(a) < CUDART_INF)) bad = 1;
+        }
+    if (__any_sync(0xffffffffu, bad) && lane_id() == 0) atomicOr(&ctrl->invalid, 1);
+}
+
 // also clears the counters (invariant of the general path: cell_cnt[] is zero between kernels that use it)
 __global__ void k_max_count(int *__restrict__ cell_cnt, int n_cell, Ctrl *ctrl)
 {
@@ -337,8 +349,9 @@ constexpr unsigned long long kFlagAggregate = 1ull << 32, kFlagInclusive = 2ull 
 
 __global__ void __launch_bounds__(kCompactThreads)
 k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
-          unsigned long long *__restrict__ status)
+          unsigned long long *__restrict__ status, const AttrView av)
 {
+    extern __shared__ double s_extra[];                // av.n rows of kCompactTile values (extra attributes)
     __shared__ int64_t s_xi[kCompactTile];
     __shared__ double s_v[kCompactTile];
     __shared__ int32_t s_c[kCompactTile];
@@ -363,6 +376,14 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
         for (int k = 0; k < kItems; ++k) {
             int e = k * kCompactThreads + tid;
             if (e < cnt) { s_xi[e] = xi[base + e]; s_v[e] = v[base + e]; s_c[e] = cell[base + e]; }
+        }
+        for (int r = 0; r < av.n; ++r) {                // staged BEFORE the tile publishes its count, like xi and v
+            const double *A = av.p + (long long)r * av.stride + base;
+#pragma unroll
+            for (int k = 0; k < kItems; ++k) {
+                int e = k * kCompactThreads + tid;
+                if (e < cnt) s_extra[r * kCompactTile + e] = A[e];
+            }
         }
         __syncthreads();
         unsigned masks[kItems];
@@ -416,6 +437,7 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
                 xi[dst] = s_xi[e];
                 v[dst] = s_v[e];
                 cell[dst] = s_c[e];
+                for (int r = 0; r < av.n; ++r) av.p[(long long)r * av.stride + dst] = s_extra[r * kCompactTile + e];
             }
             run += __popc(masks[k]);
         }

@@ -37,7 +37,7 @@ def test_no_torch_types_and_extern_c_in_header():
 
 
 def test_version_and_workspace_sizing(lib):
-    assert lib.sdm_version() == 1000
+    assert lib.sdm_version() == 1001
     assert lib.sdm_workspace_bytes(0, 1) == 0
     assert lib.sdm_workspace_bytes(10, 0) == 0
     assert lib.sdm_workspace_bytes(2 ** 31, 1) == 0
@@ -47,6 +47,11 @@ def test_version_and_workspace_sizing(lib):
     # state (20 B) + idx (4 B) + order (4 B) per droplet dominate; everything else is < 10 %
     assert 28 * 2 ** 26 <= big < 1.1 * 28 * 2 ** 26
     assert small % 256 == 0 and big % 256 == 0
+    # extensive attributes: 8 B per droplet and extra row; n_attr = 1 is the plain layout
+    assert lib.sdm_workspace_bytes_attr(1000, 4, 1) == small
+    assert lib.sdm_workspace_bytes_attr(1000, 4, 0) == 0 and lib.sdm_workspace_bytes_attr(1000, 4, 9) == 0
+    a3 = lib.sdm_workspace_bytes_attr(2 ** 20, 4, 3) - lib.sdm_workspace_bytes_attr(2 ** 20, 4, 1)
+    assert 2 * 8 * 2 ** 20 <= a3 < 2 * 8 * 2 ** 20 + 4096
 
 
 def test_create_rejects_bad_arguments_without_touching_the_gpu(lib):
@@ -58,6 +63,7 @@ def test_create_rejects_bad_arguments_without_touching_the_gpu(lib):
     assert lib.sdm_create(C.byref(h), 10, 1, C.c_void_p(256), 16, None) == -1       # too small
     assert b"workspace" in lib.sdm_last_error(None)
     assert h.value is None
+    assert lib.sdm_create_attr(C.byref(h), 10, 1, 9, C.c_void_p(256), 1 << 30, None) == -1   # n_attr > SDM_MAX_ATTR
     assert lib.sdm_destroy(None) == -1 and lib.sdm_set_option(None, 1, 1) == -1
 
 
