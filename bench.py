@@ -30,9 +30,9 @@ METRIC = "super-droplet-steps/s"
 UNIT = "sd-steps/s"
 
 # algorithmic bytes per droplet-step: compulsory traffic of the method
-B_ALG_FUSED_KERNEL = 20.0      # read xi 8 + v 8, write idx 4 (dominant kernel, cell-contiguous path)
-B_ALG_CELL_INDEX = 4.0         # read cell_id
-B_ALG_STEP = B_ALG_FUSED_KERNEL + B_ALG_CELL_INDEX   # moments ride on the same pass; remove_zero: 0 when nothing to remove
+B_ALG_FUSED_KERNEL = 24.0      # dominant kernel, cell-contiguous path: read xi 8 + v 8 + cell_id 4, write idx 4
+B_ALG_STEP = 24.0              # the whole step: the same 24 B (the cell index of the next step is derived inside the
+                               # dominant kernel; moments ride on the same pass; remove_zero: 0 when nothing to remove)
 
 
 def measured_peak_gbs():
@@ -325,7 +325,7 @@ def main():
         b_alg = B_ALG_FUSED_KERNEL if mode == 1 else None
         if b_alg is not None:
             achieved = b_alg * w.n_sd / per_launch_s / 1e9
-            roofline = {"bound": "hbm", "kernel": "k_fused_cells_count (TMA staging, Philox, per-cell counting sort, pairs, update, moments)",
+            roofline = {"bound": "hbm", "kernel": "k_fused_cells_count (TMA staging, Philox, per-cell counting sort, pairs, update, moments, next cell table from cell_id)",
                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                         "traffic": None, "peak_source": peak_src, "ms_per_launch": per_launch_s * 1e3,
                         "launches_timed": kernel_n, "alg_bytes_per_droplet": b_alg,

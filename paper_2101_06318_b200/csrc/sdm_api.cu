@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include <cuda_runtime.h>
@@ -28,7 +29,7 @@ constexpr int kMinSegCap = 8;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t xi, v, attr, cell, idx, order, cell_start, cell_cnt, cell_bits, bucket_base, bucket_start,
+    size_t xi, v, attr, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
         bucket_cnt, tile_status, part0, part1, part2, mom_out, ctrl, total;
     int64_t nb_max, n_tiles, attr_stride;
 };
@@ -48,6 +49,7 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.idx = take((size_t)cap * 4);
     L.order = take((size_t)cap * 4);
     L.cell_start = take(((size_t)n_cell + 1) * 4);
+    L.cell_start2 = take(((size_t)n_cell + 1) * 4);
     L.cell_cnt = take(((size_t)n_cell + 1) * 4);
     L.cell_bits = take(((size_t)n_cell + 1) * 4);
     L.bucket_base = take(((size_t)n_cell + 1) * 4);
@@ -79,7 +81,7 @@ struct sdm {
     int64_t *xi = nullptr;
     double *v = nullptr;
     int32_t *cell = nullptr;
-    int *idx = nullptr, *order = nullptr, *cell_start = nullptr, *cell_cnt = nullptr,
+    int *idx = nullptr, *order = nullptr, *cell_start = nullptr, *cell_start2 = nullptr, *cell_cnt = nullptr,
         *cell_bits = nullptr, *bucket_base = nullptr, *bucket_start = nullptr, *bucket_cnt = nullptr;
     unsigned long long *tile_status = nullptr;
     int64_t *part0 = nullptr;
@@ -99,6 +101,7 @@ struct sdm {
     bool force_general = false;
     int seg_cap = kWarpCap;      // fused path: largest cell; general path: only when overridden (tests)
     bool seg_cap_set = false;    // SDM_OPT_SEGMENT_CAP given
+    bool table_produced = false; // fused path: the last step's kernel wrote the next cell table into cell_start2
     bool tables_ready = false;   // general path: cell_bits / bucket_base / n_seg are valid for this state
     bool split = false;          // general path: some cell is larger than a sort segment
     int n_seg = 0;               // general path: number of sort segments when split
@@ -252,9 +255,19 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                  double *m2 = nullptr)
 {
     const int64_t n_ub = h->n_ub;
+#ifdef SDM_X_FORCE_TABLE
+    const bool produced = false;
+#else
+    const bool produced = h->table_produced;      // did the previous step's kernel leave the next cell table?
+#endif
+    h->table_produced = false;
     if (use_fused(h)) {
-        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 4 * kCellStartQuads - 1) / (4 * kCellStartQuads), 256, 32), 256, 0, h->cell, h->ctrl, h->n_cell,
-                   h->cell_start);
+        // row a2: the counting-sort kernel derives the NEXT step's table from cell_id while it runs (written
+        // to cell_start2); when it did so last step, k_cell_start_sorted only rebuilds the table if a
+        // compaction has moved droplets since (device flag), else it returns at once
+        if (produced) std::swap(h->cell_start, h->cell_start2);
+        SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 4 * kCellStartQuads - 1) / (4 * kCellStartQuads), 256, 8), 256, 0, h->cell, h->ctrl, h->n_cell,
+                   h->cell_start, produced ? 0 : 1);
         // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
         // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose
         // more to instruction fetch than they save in shuffles (measured).
@@ -265,12 +278,13 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                                     h->ctas_per_sm > 0 ? h->ctas_per_sm : kCountBlocksPerSM);
             if (m0)
                 SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
-                                        h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
-                                        h->part2, m0, m1, m2));
+                                        h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm,
+                                        h->part0, h->part1, h->part2, m0, m1, m2));
             else
                 SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<false>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
-                                        h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,
-                                        h->part2, m0, m1, m2));
+                                        h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm,
+                                        h->part0, h->part1, h->part2, m0, m1, m2));
+            h->table_produced = true;
             return SDM_OK;
         }
         int E = 8, L = 8;
@@ -370,6 +384,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
                     "state validation failed: need 0 <= cell_id < n_cell, xi >= 0, v finite and > 0");
     }
     h->valid = true;
+    h->table_produced = false;
     h->tables_ready = false;
     h->n_ub = n_sd;
     h->max_count = h->ctrl_host->max_count;
@@ -434,6 +449,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->idx = reinterpret_cast<int *>(h->ws + L.idx);
     h->order = reinterpret_cast<int *>(h->ws + L.order);
     h->cell_start = reinterpret_cast<int *>(h->ws + L.cell_start);
+    h->cell_start2 = reinterpret_cast<int *>(h->ws + L.cell_start2);
     h->cell_cnt = reinterpret_cast<int *>(h->ws + L.cell_cnt);
     h->cell_bits = reinterpret_cast<int *>(h->ws + L.cell_bits);
     h->bucket_base = reinterpret_cast<int *>(h->ws + L.bucket_base);

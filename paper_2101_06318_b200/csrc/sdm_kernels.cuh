@@ -28,7 +28,8 @@ struct Ctrl {
     unsigned int compact_done;     // compaction: CTAs that have left the kernel
     unsigned int epoch;            // compaction: tag of valid tile status words (no clearing between calls)
     int cell_ticket;               // per-cell kernel: dynamic work counter
-    int pad0[2];
+    int table_dirty;               // fused path: cell_start must be rebuilt from cell_id (set_state, or compaction moved droplets)
+    int pad0[1];
     unsigned long long n_events;   // pairs with gamma_tilde > 0
     unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
 };
@@ -274,8 +275,11 @@ __device__ __forceinline__ void cell_boundary(int prev, int c, int i, int *__res
 
 __global__ void __launch_bounds__(256)
 k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell,
-                    int *__restrict__ cell_start)
+                    int *__restrict__ cell_start, int force)
 {
+    // the previous step's kernel may already have derived this table from cell_id (sdm_fused_count.cuh,
+    // cell_table_from_staged_ids); it is stale only if a compaction has moved droplets since
+    if (!force && ctrl->table_dirty == 0) return;
     const int n = ctrl->n;
     if (n == 0) {
         for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= n_cell; c += gridDim.x * blockDim.x)
@@ -450,6 +454,7 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
         if (atomicAdd(&ctrl->compact_done, 1u) == gridDim.x - 1) {
             __threadfence();
             ctrl->n = ((volatile Ctrl *)ctrl)->n_new;
+            ctrl->table_dirty = 1;
             ctrl->zero_count = 0;
             ctrl->ticket = 0;
             ctrl->compact_done = 0;
