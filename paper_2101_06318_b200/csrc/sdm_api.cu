@@ -255,11 +255,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                  double *m2 = nullptr)
 {
     const int64_t n_ub = h->n_ub;
-#ifdef SDM_X_FORCE_TABLE
-    const bool produced = false;
-#else
     const bool produced = h->table_produced;      // did the previous step's kernel leave the next cell table?
-#endif
     h->table_produced = false;
     if (use_fused(h)) {
         // row a2: the counting-sort kernel derives the NEXT step's table from cell_id while it runs (written

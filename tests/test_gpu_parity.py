@@ -131,6 +131,38 @@ def test_c5_shape_gravitational_grid_fused(sdm_mod):
     assert events > 200
 
 
+def test_cell_table_from_the_step_kernel_survives_removals_and_empty_cells(sdm_mod):
+    """The counting-sort kernel derives the next step's cell table from cell_id; a compaction that moves
+    droplets must invalidate it (Ctrl::table_dirty).  Cells of 130..256 droplets with multiplicities 1..3:
+    droplets vanish in most steps, some cells are empty from the start, the last cells empty out."""
+    rng = np.random.default_rng(17)
+    counts = rng.integers(130, 257, 48)
+    counts[[0, 7, 8, 30, 47]] = 0
+    counts[46] = 2
+    n_cell = len(counts)
+    cell = np.repeat(np.arange(n_cell, dtype=np.int32), counts)
+    n = len(cell)
+    xi = rng.integers(1, 4, n).astype(np.int64)
+    xi[cell == 46] = 1
+    w = workloads.Workload("table", xi, np.ones(n), cell, n_cell, 1.0, 1.0, workloads.configs.KERNEL_GOLOVIN,
+                           0.002, 0, seed=5)
+    events, n_end = _run_parity(sdm_mod, w, 14, expect_mode=1)
+    assert events > 2000 and n_end < n - 500
+    # steps without any removal in between (xi large): the derived table is used as is
+    w2 = workloads.Workload("table2", xi * 1000, np.ones(n), cell, n_cell, 1.0, 1.0,
+                            workloads.configs.KERNEL_GOLOVIN, 1e-6, 0, seed=6)
+    s = _make(sdm_mod, w2)
+    x2, v2, c2 = w2.xi.copy(), w2.v.copy(), w2.cell_id.copy()
+    for step in range(5):
+        s.remove_zero(sync=False)
+        s.coalescence_step(w2.dt, w2.dV, w2.kernel, w2.kparam, w2.seed, step)
+        idx, cs, _ = oracle.step(x2, v2, c2, n_cell, w2.dt, w2.dV, w2.kernel, w2.kparam, w2.seed, step)
+        gidx, gcs = (t.cpu().numpy() for t in s.get_permutation(n))
+        assert np.array_equal(gcs, cs) and np.array_equal(gidx, idx)
+    assert np.array_equal(s.get_state()[0].cpu().numpy(), x2)
+    s.close()
+
+
 # ---- ragged, degenerate and maximum-size segments --------------------------------------------------
 
 def _ragged_workload(counts, seed=0, shuffled=False, kparam=0.002):
