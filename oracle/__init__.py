@@ -15,6 +15,7 @@ from .build import build as _build
 
 KERNEL_GOLOVIN = 0
 KERNEL_GRAVITATIONAL = 1
+KERNEL_GRAVITATIONAL_TABULATED = 2
 
 _lib = None
 
@@ -37,6 +38,10 @@ def lib() -> C.CDLL:
         L.orc_cbrt_spec.restype = C.c_double
         L.orc_kernel.argtypes = [C.c_int32, C.c_double, C.c_double, C.c_double]
         L.orc_kernel.restype = C.c_double
+        L.orc_set_efficiency_table.argtypes = [C.c_int32, p, p]
+        L.orc_set_efficiency_table.restype = C.c_int
+        L.orc_efficiency.argtypes = [C.c_double, C.c_double]
+        L.orc_efficiency.restype = C.c_double
         L.orc_pair_probability.argtypes = [C.c_double, C.c_int64, C.c_int64, C.c_double, C.c_double]
         L.orc_pair_probability.restype = C.c_double
         L.orc_gamma_tilde.argtypes = [C.c_double, C.c_double, C.c_int64, C.c_int64]
@@ -111,6 +116,19 @@ def cbrt_spec(x: float) -> float:
 
 def kernel(ktype: int, kparam: float, vj: float, vk: float) -> float:
     return lib().orc_kernel(ktype, float(kparam), float(vj), float(vk))
+
+
+def set_efficiency_table(r_grid, E):
+    """Collection-efficiency table of KERNEL_GRAVITATIONAL_TABULATED: E[n_r, n_r] on the radius grid r_grid."""
+    r_grid = _chk(np.ascontiguousarray(r_grid, dtype=np.float64), np.float64)
+    E = _chk(np.ascontiguousarray(E, dtype=np.float64), np.float64)
+    assert E.shape == (r_grid.shape[0], r_grid.shape[0])
+    if lib().orc_set_efficiency_table(r_grid.shape[0], _ptr(r_grid), _ptr(E)) != 0:
+        raise ValueError("invalid efficiency table")
+
+
+def efficiency(rj: float, rk: float) -> float:
+    return lib().orc_efficiency(float(rj), float(rk))
 
 
 def pair_probability(K: float, xi_max: int, n_s: int, dt: float, dV: float) -> float:

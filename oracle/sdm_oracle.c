@@ -145,6 +145,62 @@ static double orc_terminal_velocity(double r)
     return 220.0 * sqrt(r);
 }
 
+/* NEXT-2 ("potentially user-supplied kernel code", kernels "after Berry 1967" with
+ * collection efficiencies): a user-supplied collection-efficiency table E(r_1, r_2) on a rectangular radius
+ * grid r_0 < r_1 < ... < r_{n-1}, bilinear in (r_1, r_2), clamped outside the grid (R16).
+ * One table per process: the oracle is single-threaded test infrastructure. */
+static int32_t orc_eff_n = 0;
+static double *orc_eff_grid = NULL, *orc_eff_tab = NULL;
+
+int orc_set_efficiency_table(int32_t n_r, const double *r_grid, const double *E)
+{
+    if (n_r < 2 || !r_grid || !E) return -1;
+    for (int32_t i = 0; i < n_r; ++i) {
+        if (!(r_grid[i] > 0.0) || !isfinite(r_grid[i])) return -1;
+        if (i > 0 && !(r_grid[i] > r_grid[i - 1])) return -1;
+    }
+    for (int64_t i = 0; i < (int64_t)n_r * n_r; ++i)
+        if (!(E[i] >= 0.0) || !isfinite(E[i])) return -1;
+    free(orc_eff_grid); free(orc_eff_tab);
+    orc_eff_grid = (double *)malloc((size_t)n_r * sizeof(double));
+    orc_eff_tab = (double *)malloc((size_t)n_r * n_r * sizeof(double));
+    memcpy(orc_eff_grid, r_grid, (size_t)n_r * sizeof(double));
+    memcpy(orc_eff_tab, E, (size_t)n_r * n_r * sizeof(double));
+    orc_eff_n = n_r;
+    return 0;
+}
+
+/* grid interval of r and the weight inside it: i in [0, n-2], t in [0, 1] */
+static void orc_eff_locate(double r, int32_t *i_out, double *t_out)
+{
+    const int32_t n = orc_eff_n;
+    if (r < orc_eff_grid[0]) { *i_out = 0; *t_out = 0.0; return; }
+    if (r >= orc_eff_grid[n - 1]) { *i_out = n - 2; *t_out = 1.0; return; }
+    int32_t i = 0;
+    while (orc_eff_grid[i + 1] <= r) ++i;             /* grid[i] <= r < grid[i+1] */
+    double num = r - orc_eff_grid[i];
+    double den = orc_eff_grid[i + 1] - orc_eff_grid[i];
+    *i_out = i;
+    *t_out = num / den;
+}
+
+double orc_efficiency(double rj, double rk)
+{
+    int32_t i, k;
+    double t, u;
+    orc_eff_locate(rj, &i, &t);
+    orc_eff_locate(rk, &k, &u);
+    const int32_t n = orc_eff_n;
+    double e00 = orc_eff_tab[(int64_t)i * n + k], e10 = orc_eff_tab[(int64_t)(i + 1) * n + k];
+    double e01 = orc_eff_tab[(int64_t)i * n + k + 1], e11 = orc_eff_tab[(int64_t)(i + 1) * n + k + 1];
+    double d0 = e10 - e00;
+    double e0 = e00 + t * d0;                         /* along r_j at r-grid column k   */
+    double d1 = e11 - e01;
+    double e1 = e01 + t * d1;                         /* along r_j at column k+1         */
+    double d = e1 - e0;
+    return e0 + u * d;                                /* along r_k                       */
+}
+
 double orc_kernel(int32_t type, double kparam, double vj, double vk)
 {
     if (type == ORC_KERNEL_GOLOVIN) {
@@ -161,7 +217,9 @@ double orc_kernel(int32_t type, double kparam, double vj, double vk)
     double wk = orc_terminal_velocity(rk);
     double s = rj + rk;
     double s2 = s * s;
-    double K = kparam * pi;
+    double E = kparam;
+    if (type == ORC_KERNEL_GRAVITATIONAL_TABULATED) E = kparam * orc_efficiency(rj, rk);
+    double K = E * pi;
     K = K * s2;
     K = K * fabs(wj - wk);
     return K;

@@ -25,7 +25,7 @@
 extern "C" {
 #endif
 
-enum { ORC_KERNEL_GOLOVIN = 0, ORC_KERNEL_GRAVITATIONAL = 1 };
+enum { ORC_KERNEL_GOLOVIN = 0, ORC_KERNEL_GRAVITATIONAL = 1, ORC_KERNEL_GRAVITATIONAL_TABULATED = 2 };
 
 /* Philox4x32-10 (Salmon et al. 2011), one block.  DESIGN.md R6. */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
@@ -49,6 +49,13 @@ double orc_cbrt_spec(double x);
 /* Coalescence kernel a(v_j, v_k) [m^3/s]: Golovin b*(v_j+v_k) or the
  * gravitational kernel of BASELINE.json config 3 (PAPER.md:326 gives no formula). */
 double orc_kernel(int32_t type, double kparam, double vj, double vk);
+
+/* NEXT-2: user-supplied collection efficiency E(r_1, r_2) for ORC_KERNEL_GRAVITATIONAL_TABULATED
+ * (a = kparam * E(r_j, r_k) * pi * (r_j + r_k)^2 * |w_j - w_k|): n_r x n_r table,
+ * row-major, on the strictly increasing radius grid r_grid; bilinear, clamped outside (R16).
+ * Returns 0, -1 on an invalid table.  The table is copied. */
+int orc_set_efficiency_table(int32_t n_r, const double *r_grid, const double *E);
+double orc_efficiency(double rj, double rk);
 
 /* Eq. 3, evaluated in the routine order of Fig. 3. */
 double orc_pair_probability(double K, int64_t xi_max, int64_t n_s, double dt, double dV);
