@@ -36,13 +36,15 @@ typedef struct sdm sdm_t; /* opaque handle, owned by the library (host memory on
 enum { SDM_OK = 0, SDM_EINVAL = -1, SDM_ECAPACITY = -2, SDM_ECUDA = -3, SDM_ESTATE = -4 };
 
 /* Coalescence kernel a(v1, v2) of Eq. 1 / Eq. 3. */
-enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GRAVITATIONAL = 1 };
+enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GRAVITATIONAL = 1, SDM_KERNEL_GRAVITATIONAL_TABULATED = 2 };
 typedef struct {
     int32_t type;     /* SDM_KERNEL_*                                                              */
     int32_t reserved; /* must be 0                                                                 */
     double b;         /* Golovin: a = b*(v1+v2), b in 1/s                           */
     double E;         /* gravitational: a = E*pi*(r1+r2)^2*|w(r1)-w(r2)|, collection efficiency E  */
                       /* (constants of BASELINE.json config 3, R9-R10)      */
+                      /* tabulated: a = E*Etab(r1,r2)*pi*(r1+r2)^2*|w(r1)-w(r2)|, Etab from              */
+                      /* sdm_set_efficiency_table                                                     */
 } sdm_kernel_t;
 
 /* Options for sdm_set_option (testing / profiling; defaults in brackets). */
@@ -118,6 +120,17 @@ int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld);
 
 /* Copies rows 1 .. n_attr-1 out (row r to attr_dev + (r-1)*ld, current n_sd values each).  SYNCHRONOUS. */
 int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld);
+
+/* User-supplied collection efficiencies for SDM_KERNEL_GRAVITATIONAL_TABULATED (the paper separates the
+ * pair logic from "potentially user-supplied kernel code", and takes its kernels with their
+ * efficiencies from tables after Berry 1967): E_host[n_r * n_r], row-major, E_host[i*n_r + k] =
+ * efficiency for radii (r_grid_host[i], r_grid_host[k]), on a strictly increasing grid of positive radii [m],
+ * 2 <= n_r <= SDM_MAX_EFF_GRID; all values finite and >= 0.  Between grid points the table is interpolated
+ * bilinearly (first along the radius of the droplet with the larger multiplicity, every operation rounded),
+ * outside the grid it is clamped (R16).  Both arrays are HOST pointers and are copied into the
+ * workspace; SYNCHRONOUS.  The table stays until replaced; it is independent of the loaded state. */
+#define SDM_MAX_EFF_GRID 64
+int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host);
 
 /* Copies the current state out in storage order.  Any of the array pointers may be NULL.
  * SYNCHRONOUS (returns n_sd on the host).  The arrays must hold at least n_sd elements (capacity

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     SdmError,
     KERNEL_GOLOVIN,
     KERNEL_GRAVITATIONAL,
+    KERNEL_GRAVITATIONAL_TABULATED,
     OPT_FORCE_GENERAL,
     OPT_SEGMENT_CAP,
     OPT_WRITE_IDX,

@@ -12,6 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 KERNEL_GOLOVIN = 0
 KERNEL_GRAVITATIONAL = 1
+KERNEL_GRAVITATIONAL_TABULATED = 2
 OPT_FORCE_GENERAL = 1
 OPT_SEGMENT_CAP = 2
 OPT_WRITE_IDX = 3
@@ -33,6 +34,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
+    "sdm_set_efficiency_table",
 )
 MAX_ATTR = 8
 
@@ -75,6 +77,7 @@ def load_library() -> C.CDLL:
     L.sdm_create_attr.argtypes = [C.POINTER(vp), i64, i32, i32, vp, C.c_size_t, vp]
     L.sdm_set_attributes.argtypes = [vp, vp, i64]
     L.sdm_get_attributes.argtypes = [vp, vp, i64]
+    L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
     L.sdm_set_state.argtypes = [vp, i64, vp, vp, vp]
@@ -186,6 +189,16 @@ class SDM:
         n = xi.shape[0]
         self._host(xi, t.int64), self._host(v, t.float64), self._host(cell_id, t.int32)
         self._check(self._lib.sdm_set_state_host(self._h, n, self._p(xi), self._p(v), self._p(cell_id)))
+
+    def set_efficiency_table(self, r_grid, E):
+        """Collection efficiencies for KERNEL_GRAVITATIONAL_TABULATED: numpy float64 r_grid[n_r], E[n_r, n_r]."""
+        import numpy as np
+
+        r_grid = np.ascontiguousarray(r_grid, dtype=np.float64)
+        E = np.ascontiguousarray(E, dtype=np.float64)
+        assert E.shape == (r_grid.shape[0], r_grid.shape[0])
+        self._check(self._lib.sdm_set_efficiency_table(self._h, int(r_grid.shape[0]), r_grid.ctypes.data_as(C.c_void_p),
+                                                       E.ctypes.data_as(C.c_void_p)))
 
     def set_attributes(self, attr):
         """Rows 1..n_attr-1 of the attribute block: a contiguous float64 device tensor [n_attr-1, n_sd]."""

@@ -29,7 +29,7 @@ constexpr int kMinSegCap = 8;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t xi, v, attr, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
+    size_t xi, v, attr, eff, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
         bucket_cnt, tile_status, part0, part1, part2, mom_out, ctrl, total;
     int64_t nb_max, n_tiles, attr_stride;
 };
@@ -61,6 +61,7 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.part2 = take((size_t)kMomentBlocks * 8);
     L.mom_out = take(3 * 8);
     L.ctrl = take(sizeof(Ctrl));
+    L.eff = take((size_t)(SDM_MAX_EFF_GRID + SDM_MAX_EFF_GRID * SDM_MAX_EFF_GRID) * 8);   // efficiency grid + table
     L.total = off;
     return L;
 }
@@ -74,6 +75,9 @@ struct sdm {
     int32_t n_cell = 0;
     int32_t n_attr = 1;          // extensive attributes per droplet, volume included
     double *attr = nullptr;      // rows 1..n_attr-1
+    double *eff = nullptr;       // efficiency grid [SDM_MAX_EFF_GRID] followed by the table
+    int eff_n = 0;               // 0: no table loaded
+    double eff_max = 0.0;        // largest table entry (screening bounds)
     cudaStream_t stream = nullptr;
     unsigned char *ws = nullptr;
     Layout L{};
@@ -194,6 +198,9 @@ AttrView attr_view(const sdm_t *h)
     av.p = h->attr;
     av.stride = h->L.attr_stride;
     av.n = h->n_attr - 1;
+    av.eff_n = h->eff_n;
+    av.eff_grid = h->eff;
+    av.eff_tab = h->eff + SDM_MAX_EFF_GRID;
     return av;
 }
 
@@ -210,14 +217,18 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     if (!kernel) return fail(h, SDM_EINVAL, "kernel is NULL");
     if (!(dt >= 0.0) || !(dV > 0.0) || !std::isfinite(dt) || !std::isfinite(dV))
         return fail(h, SDM_EINVAL, "need dt >= 0 and dV > 0, both finite");
-    if (kernel->type != SDM_KERNEL_GOLOVIN && kernel->type != SDM_KERNEL_GRAVITATIONAL)
+    if (kernel->type != SDM_KERNEL_GOLOVIN && kernel->type != SDM_KERNEL_GRAVITATIONAL &&
+        kernel->type != SDM_KERNEL_GRAVITATIONAL_TABULATED)
         return fail(h, SDM_EINVAL, "unknown kernel type");
+    if (kernel->type == SDM_KERNEL_GRAVITATIONAL_TABULATED && h->eff_n < 2)
+        return fail(h, SDM_EINVAL, "SDM_KERNEL_GRAVITATIONAL_TABULATED needs sdm_set_efficiency_table first");
     if (kernel->reserved != 0) return fail(h, SDM_EINVAL, "kernel.reserved must be 0");
     double kp = kernel->type == SDM_KERNEL_GOLOVIN ? kernel->b : kernel->E;
     if (!std::isfinite(kp) || kp < 0.0) return fail(h, SDM_EINVAL, "kernel parameter must be finite and >= 0");
     prm = StepParams{};
     prm.dtdv = dt / dV;
     prm.kparam = kp;
+    prm.kparam_ub = kernel->type == SDM_KERNEL_GRAVITATIONAL_TABULATED ? kp * h->eff_max : kp;
     prm.kernel = kernel->type;
     prm.write_idx = h->write_idx ? 1 : 0;
     prm.seed = seed;
@@ -272,14 +283,16 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         if (bucket) {
             const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32,
                                     h->ctas_per_sm > 0 ? h->ctas_per_sm : kCountBlocksPerSM);
-            if (m0)
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<true>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
-                                        h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm,
-                                        h->part0, h->part1, h->part2, m0, m1, m2));
-            else
-                SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<false>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,
-                                        h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm,
-                                        h->part0, h->part1, h->part2, m0, m1, m2));
+#define SDM_COUNT(MM, TT)                                                                                      \
+    SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<MM, TT>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,  \
+                            h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm, h->part0,    \
+                            h->part1, h->part2, m0, m1, m2))
+            const bool tab = prm.kernel == SDM_KERNEL_GRAVITATIONAL_TABULATED;
+            if (m0 && tab) SDM_COUNT(true, true);
+            else if (m0) SDM_COUNT(true, false);
+            else if (tab) SDM_COUNT(false, true);
+            else SDM_COUNT(false, false);
+#undef SDM_COUNT
             h->table_produced = true;
             return SDM_OK;
         }
@@ -392,7 +405,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
 
 extern "C" {
 
-int sdm_version(void) { return 1001; }
+int sdm_version(void) { return 1002; }
 
 size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
@@ -441,6 +454,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->xi = reinterpret_cast<int64_t *>(h->ws + L.xi);
     h->v = reinterpret_cast<double *>(h->ws + L.v);
     h->attr = reinterpret_cast<double *>(h->ws + L.attr);
+    h->eff = reinterpret_cast<double *>(h->ws + L.eff);
     h->cell = reinterpret_cast<int32_t *>(h->ws + L.cell);
     h->idx = reinterpret_cast<int *>(h->ws + L.idx);
     h->order = reinterpret_cast<int *>(h->ws + L.order);
@@ -469,10 +483,11 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
     e = cudaFuncSetAttribute(k_segment_sort_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_pairs)");
-    e = cudaFuncSetAttribute(k_fused_cells_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<true>)");
-    e = cudaFuncSetAttribute(k_fused_cells_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
-    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count<false>)");
+    e = cudaFuncSetAttribute(k_fused_cells_count<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count)");
     if (n_attr > 1) {
         e = cudaFuncSetAttribute(k_compact, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)((SDM_MAX_ATTR - 1) * kCompactTile * 8));
@@ -565,6 +580,29 @@ int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const dou
         SDM_CUDA(h, cudaMemcpyAsync(h->cell, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, h->stream));
     }
     return load_state_common(h, n_sd);
+}
+
+int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host)
+{
+    if (!h) return SDM_EINVAL;
+    if (n_r < 2 || n_r > SDM_MAX_EFF_GRID) return fail(h, SDM_EINVAL, "need 2 <= n_r <= SDM_MAX_EFF_GRID");
+    if (!r_grid_host || !E_host) return fail(h, SDM_EINVAL, "table pointer is NULL");
+    for (int i = 0; i < n_r; ++i) {
+        if (!(r_grid_host[i] > 0.0) || !std::isfinite(r_grid_host[i]) || (i > 0 && !(r_grid_host[i] > r_grid_host[i - 1])))
+            return fail(h, SDM_EINVAL, "radius grid must be positive, finite and strictly increasing");
+    }
+    double emax = 0.0;
+    for (int i = 0; i < n_r * n_r; ++i) {
+        if (!(E_host[i] >= 0.0) || !std::isfinite(E_host[i])) return fail(h, SDM_EINVAL, "efficiencies must be finite and >= 0");
+        emax = std::fmax(emax, E_host[i]);
+    }
+    SDM_CUDA(h, cudaStreamSynchronize(h->stream));      // steps that still read the old table
+    SDM_CUDA(h, cudaMemcpyAsync(h->eff, r_grid_host, (size_t)n_r * 8, cudaMemcpyHostToDevice, h->stream));
+    SDM_CUDA(h, cudaMemcpyAsync(h->eff + SDM_MAX_EFF_GRID, E_host, (size_t)n_r * n_r * 8, cudaMemcpyHostToDevice, h->stream));
+    SDM_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->eff_n = n_r;
+    h->eff_max = emax;
+    return SDM_OK;
 }
 
 int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld)

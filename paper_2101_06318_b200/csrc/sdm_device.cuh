@@ -72,12 +72,17 @@ struct AttrView {
     double *p;
     long long stride;
     int n;                  // number of extra rows (0: volume is the only attribute)
-    int pad;
+    // NEXT-2 rides in the same per-pair bundle: the user's collection-efficiency table of
+    // SDM_KERNEL_GRAVITATIONAL_TABULATED (R16): eff_tab[eff_n][eff_n] on the radius grid eff_grid[eff_n]
+    int eff_n;
+    const double *eff_grid;
+    const double *eff_tab;
 };
 
 struct StepParams {
     double dtdv;      // dt / dV, one IEEE division on the host
     double kparam;    // Golovin b, or gravitational E
+    double kparam_ub; // upper bound of kparam times the efficiency table's maximum (screening bounds only)
     int32_t kernel;   // SDM_KERNEL_*
     int32_t write_idx;
     uint64_t seed, step;
@@ -116,6 +121,33 @@ __device__ __forceinline__ double terminal_velocity(double r)
     return __dmul_rn(220.0, __dsqrt_rn(r));
 }
 
+// R16: bilinear interpolation of the efficiency table, clamped outside the grid; every operation rounded
+__device__ __forceinline__ void efficiency_locate(const double *__restrict__ grid, int n, double r, int &i, double &t)
+{
+    if (r < grid[0]) { i = 0; t = 0.0; return; }
+    if (r >= grid[n - 1]) { i = n - 2; t = 1.0; return; }
+    int lo = 0, hi = n - 1;                                             // grid[lo] <= r < grid[hi]
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (grid[mid] <= r) lo = mid; else hi = mid;
+    }
+    i = lo;
+    t = __ddiv_rn(__dsub_rn(r, grid[lo]), __dsub_rn(grid[lo + 1], grid[lo]));
+}
+
+__device__ __forceinline__ double collection_efficiency(const AttrView &av, double rj, double rk)
+{
+    int i, k;
+    double t, u;
+    efficiency_locate(av.eff_grid, av.eff_n, rj, i, t);
+    efficiency_locate(av.eff_grid, av.eff_n, rk, k, u);
+    const double *row0 = av.eff_tab + (long long)i * av.eff_n + k, *row1 = row0 + av.eff_n;
+    const double e00 = row0[0], e01 = row0[1], e10 = row1[0], e11 = row1[1];
+    const double e0 = __dadd_rn(e00, __dmul_rn(t, __dsub_rn(e10, e00)));
+    const double e1 = __dadd_rn(e01, __dmul_rn(t, __dsub_rn(e11, e01)));
+    return __dadd_rn(e0, __dmul_rn(u, __dsub_rn(e1, e0)));
+}
+
 __device__ __forceinline__ double coalescence_kernel(int32_t type, double kparam, double vj, double vk)
 {
     if (type == 0) return __dmul_rn(kparam, __dadd_rn(vj, vk));       // Golovin
@@ -126,6 +158,20 @@ __device__ __forceinline__ double coalescence_kernel(int32_t type, double kparam
     double wj = terminal_velocity(rj), wk = terminal_velocity(rk);
     double s = __dadd_rn(rj, rk);
     double K = __dmul_rn(kparam, pi);
+    K = __dmul_rn(K, __dmul_rn(s, s));
+    return __dmul_rn(K, fabs(__dsub_rn(wj, wk)));
+}
+
+// NEXT-2, SDM_KERNEL_GRAVITATIONAL_TABULATED: the gravitational kernel with E = kparam * Etab(r_j, r_k).
+__device__ __noinline__ double coalescence_kernel_tabulated(double kparam, double vj, double vk, const AttrView &av)
+{
+    const double c = 0x1.e8ec8a4aeacc4p-3;                              // 3/(4 pi)
+    const double pi = 0x1.921fb54442d18p+1;
+    double rj = cbrt_spec(__dmul_rn(vj, c));
+    double rk = cbrt_spec(__dmul_rn(vk, c));
+    double wj = terminal_velocity(rj), wk = terminal_velocity(rk);
+    double s = __dadd_rn(rj, rk);
+    double K = __dmul_rn(__dmul_rn(kparam, collection_efficiency(av, rj, rk)), pi);
     K = __dmul_rn(K, __dmul_rn(s, s));
     return __dmul_rn(K, fabs(__dsub_rn(wj, wk)));
 }
@@ -141,7 +187,11 @@ __device__ __forceinline__ double pair_norm(int n_s, double dtdv)
 // ---------------------------------------------------------------------------------------------
 // Rows a5-a6 for one candidate pair (a = first-in-pair, b = second), in place in global memory.
 // Returns bit 0: an event happened (gamma_tilde > 0); bit 1: a multiplicity became zero.
+// TAB: the kernel type may be SDM_KERNEL_GRAVITATIONAL_TABULATED.  The dominant kernel is instantiated without
+// it for the built-in kernels: it runs at its register limit, and the mere presence of the table code in its
+// call graph cost 10 % (measured: 0.383 -> 0.421 ms on C5).
 // ---------------------------------------------------------------------------------------------
+template <bool TAB>
 __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, double *__restrict__ v,
                                                   int a, int b, double u, double norm,
                                                   int32_t ktype, double kparam, const AttrView &av)
@@ -152,7 +202,8 @@ __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, doub
     if (xa < xb) { j = b; k = a; xj = xb; xk = xa; }     // PAPER.md:257-259 (strict <, R8)
     if (xk == 0) return 0;                               // R11
     double vj = v[j], vk = v[k];
-    double K = coalescence_kernel(ktype, kparam, vj, vk);
+    double K = (TAB && ktype == 2) ? coalescence_kernel_tabulated(kparam, vj, vk, av)
+                                   : coalescence_kernel(ktype, kparam, vj, vk);
     double p = __dmul_rn(__dmul_rn(K, __ll2double_rn(xj)), norm);      // Eq. 3 in routine order (R3)
     double fl = floor(p);
     int64_t q = xj / xk;

@@ -163,6 +163,7 @@ __device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v,
 // sk: the group's sorted words; sflag[k]: ballot word of element slot k (bit = lane of the warp);
 // lane0: first lane of the group.  delta (may be NULL): three doubles per lane receiving the change
 // of (M0, M1, M2) caused by this lane's events (M0's change as the bit pattern of an int64).
+template <bool TAB>
 __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int L, int lane0,
                                             int64_t *xi, double *v, int s, int n_s, int li, double dtdv,
                                             int32_t ktype, double kparam, uint64_t seed, uint64_t step,
@@ -185,7 +186,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
         int64_t o0 = 0;
         double o1 = 0.0, o2 = 0.0;
         if (delta) pair_moments(xi, v, s + a, s + b, o0, o1, o2);
-        const int r = collide_pair_exact(xi, v, s + a, s + b, u, norm, ktype, kparam, av);
+        const int r = collide_pair_exact<TAB>(xi, v, s + a, s + b, u, norm, ktype, kparam, av);
         if (delta && (r & 1)) {
             int64_t n0;
             double n1, n2;
@@ -206,6 +207,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 
 // Cells larger than the kernel's capacity cannot reach it (the host checks the largest cell at
 // sdm_set_state and cells never grow); this keeps the result defined anyway.  Whole warp, one cell.
+template <bool TAB>
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
                                           double dtdv, int32_t ktype, double kparam, uint64_t seed,
                                           uint64_t step, double *delta, const AttrView &av)
@@ -219,7 +221,7 @@ __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int 
     for (int q = lane; q < (n_s >> 1); q += 32) {
         int a = idx[s + 2 * q], b = idx[s + 2 * q + 1];
         double u = block_uniform(droplet_block((uint32_t)a, step, rk));
-        int r = collide_pair_exact(xi, v, a, b, u, norm, ktype, kparam, av);
+        int r = collide_pair_exact<TAB>(xi, v, a, b, u, norm, ktype, kparam, av);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
     if (delta) {                                      // here: the cell's whole post-step contribution
@@ -281,7 +283,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             for (int gg = 0; gg < G; ++gg) {
                 const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
                 if (n2 <= N) continue;
-                const int pk = oversize_cell(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
+                const int pk = oversize_cell<true>(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
                                              prm.seed, prm.step, my_delta, prm.attr);
                 events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
                 if (MOM) {
@@ -323,7 +325,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         uint32_t thr = 0xFFFFFFFFu;
         if (prm.screening) {
             const double v_ub = __hiloint2double((int)(vhi_max + 1u), 0);
-            const double P = cell_probability_bound(prm.kernel, prm.kparam, v_ub, (double)xi_max,
+            const double P = cell_probability_bound(prm.kernel, prm.kparam_ub, v_ub, (double)xi_max,
                                                     pair_norm(n_s, prm.dtdv));
             thr = flag_threshold(P);
         }
@@ -395,7 +397,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
 #pragma unroll
             for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
             __syncwarp();
-            const int pk = collide_flagged(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
+            const int pk = collide_flagged<true>(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
                                            prm.kernel, prm.kparam, prm.seed, prm.step, my_delta, prm.attr);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
             if (MOM) {

@@ -221,7 +221,7 @@ __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, in
     for (int e = ((s - cs) & 1) + 2 * lane; e + 1 < m; e += 64) {
         const int a = sorted[e], b = sorted[e + 1];
         const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
-        const int r = collide_pair_exact(xi, v, a, b, u, norm, prm.kernel, prm.kparam, prm.attr);
+        const int r = collide_pair_exact<true>(xi, v, a, b, u, norm, prm.kernel, prm.kparam, prm.attr);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
     return packed;
@@ -341,7 +341,7 @@ k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__rest
         const int cs = cell_start[c];
         if ((p - 1 - cs) & 1) continue;                    // a is a second-in-pair
         const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
-        const int r = collide_pair_exact(xi, v, a, b, u, pair_norm(cell_start[c + 1] - cs, prm.dtdv), prm.kernel,
+        const int r = collide_pair_exact<true>(xi, v, a, b, u, pair_norm(cell_start[c + 1] - cs, prm.dtdv), prm.kernel,
                                          prm.kparam, prm.attr);
         events += r & 1;
         zeros += (r >> 1) & 1;
