@@ -53,6 +53,8 @@ def lib() -> C.CDLL:
         L.orc_step.restype = C.c_int
         L.orc_remove_zero.argtypes = [C.c_int64, p, p, p]
         L.orc_remove_zero.restype = C.c_int64
+        L.orc_spectrum.argtypes = [C.c_int64, p, p, C.c_int32, p, p, C.c_double, C.c_double, C.c_int32, p]
+        L.orc_spectrum.restype = None
         L.orc_collide_pair_attr.argtypes = [p, p, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int64]
         L.orc_collide_pair_attr.restype = None
         L.orc_step_attr.argtypes = [C.c_int64, p, p, C.c_int32, C.c_int64, p, C.c_int32, p, C.c_double, C.c_double,
@@ -227,3 +229,17 @@ def moments(xi, v, cell_id=None, n_cell=1, per_cell=False):
     if per_cell:
         return m0, m1, m2
     return int(m0[0]), float(m1[0]), float(m2[0])
+
+
+def spectrum(xi, v, v_edges, dlnr, rho, V, n_smooth=2):
+    """Mass density per unit ln r on the bins v_edges (R17)."""
+    xi = _chk(xi, np.int64)
+    v = _chk(v, np.float64)
+    v_edges = _chk(np.ascontiguousarray(v_edges, dtype=np.float64), np.float64)
+    dlnr = _chk(np.ascontiguousarray(dlnr, dtype=np.float64), np.float64)
+    nb = dlnr.shape[0]
+    assert v_edges.shape[0] == nb + 1
+    out = np.zeros(nb, dtype=np.float64)
+    lib().orc_spectrum(xi.shape[0], _ptr(xi), _ptr(v), nb, _ptr(v_edges), _ptr(dlnr), float(rho), float(V),
+                       int(n_smooth), _ptr(out))
+    return out

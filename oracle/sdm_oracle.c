@@ -397,3 +397,41 @@ void orc_moments(int64_t n, const int64_t *xi, const double *v, const int32_t *c
     for (int32_t c = 0; c < nout; ++c) { m1[c] += c1[c]; m2[c] += c2[c]; }
     free(c1); free(c2);
 }
+
+/* NEXT-3 (Fig. 6): "the mass of droplets per unit of ln r ... aggregating super-particle
+ * multiplicities onto a grid of ca. 100 bins, and smoothing the result twice with a running average with a
+ * centered window spanning five bins".  Readings (R17): bin b holds the droplets with
+ * v_edges[b] <= v < v_edges[b+1]; its value is (sum xi*v) * rho / V / dlnr[b]  [kg m^-3 per unit ln r], the
+ * bin widths dlnr[b] = ln(r_{b+1}/r_b) being an INPUT (so that no logarithm has to agree between
+ * implementations); each smoothing pass replaces a bin by the mean of the bins b-2..b+2 that exist (the
+ * window is truncated at the ends), summed left to right. */
+void orc_spectrum(int64_t n, const int64_t *xi, const double *v, int32_t n_bins, const double *v_edges,
+                  const double *dlnr, double rho, double V, int32_t n_smooth, double *out)
+{
+    double *comp = (double *)calloc((size_t)n_bins, sizeof(double));
+    double *tmp = (double *)calloc((size_t)n_bins, sizeof(double));
+    for (int32_t b = 0; b < n_bins; ++b) out[b] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(v[i] >= v_edges[0]) || !(v[i] < v_edges[n_bins])) continue;
+        int32_t b = 0;
+        while (v_edges[b + 1] <= v[i]) ++b;           /* v_edges[b] <= v < v_edges[b+1] */
+        double m = (double)xi[i] * v[i];
+        orc_acc(&out[b], &comp[b], m);
+    }
+    for (int32_t b = 0; b < n_bins; ++b) {
+        double s = out[b] + comp[b];
+        s = s * rho;
+        s = s / V;
+        out[b] = s / dlnr[b];
+    }
+    for (int32_t pass = 0; pass < n_smooth; ++pass) {
+        for (int32_t b = 0; b < n_bins; ++b) {
+            int32_t lo = b - 2 < 0 ? 0 : b - 2, hi = b + 2 > n_bins - 1 ? n_bins - 1 : b + 2;
+            double s = 0.0;
+            for (int32_t k = lo; k <= hi; ++k) s = s + out[k];
+            tmp[b] = s / (double)(hi - lo + 1);
+        }
+        memcpy(out, tmp, (size_t)n_bins * sizeof(double));
+    }
+    free(comp); free(tmp);
+}

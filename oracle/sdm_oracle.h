@@ -99,6 +99,12 @@ int64_t orc_remove_zero(int64_t n, int64_t *xi, double *v, int32_t *cell_id);
 void orc_moments(int64_t n, const int64_t *xi, const double *v, const int32_t *cell_id,
                  int32_t n_cell, int32_t per_cell, int64_t *m0, double *m1, double *m2);
 
+/* NEXT-3: binned mass density per unit ln r, out[n_bins]; bins by volume edges
+ * v_edges[n_bins+1] (strictly increasing), widths dlnr[n_bins], n_smooth passes of a centered 5-bin running
+ * mean truncated at the ends (R17). */
+void orc_spectrum(int64_t n, const int64_t *xi, const double *v, int32_t n_bins, const double *v_edges,
+                  const double *dlnr, double rho, double V, int32_t n_smooth, double *out);
+
 #ifdef __cplusplus
 }
 #endif

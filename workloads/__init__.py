@@ -13,6 +13,7 @@ from .configs import (  # noqa: F401
     grid_uniform,
     grid_small_multiplicity,
     make,
+    spectrum_bins,
     V_MEAN_BOX,
     V_MEAN_C5,
 )

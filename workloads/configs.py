@@ -125,6 +125,17 @@ def grid_small_multiplicity(nx: int = 64, ny: int = 64, per_cell: int = 32, step
                     xi, v, np.ascontiguousarray(cell), n_cell, 1.0, 1.0, KERNEL_GOLOVIN, 0.01, steps)
 
 
+def spectrum_bins(n_bins: int = 100, r_min: float = 1e-6, r_max: float = 5e-3):
+    """Fig. 6's grid ("ca. 100 bins"; the range is not given): n_bins bins equally spaced in ln r.
+    Returns (v_edges[n_bins+1], dlnr[n_bins], r_mid[n_bins]); plain input data for both implementations."""
+    ln_edges = np.linspace(math.log(r_min), math.log(r_max), n_bins + 1)
+    r_edges = np.exp(ln_edges)
+    v_edges = (4.0 * math.pi / 3.0) * r_edges ** 3
+    dlnr = np.diff(ln_edges)
+    r_mid = np.exp(0.5 * (ln_edges[1:] + ln_edges[:-1]))
+    return np.ascontiguousarray(v_edges), np.ascontiguousarray(dlnr), r_mid
+
+
 def make(name: str, **kw) -> Workload:
     """Named access used by bench.py and the tests: C1..C6."""
     table = {
