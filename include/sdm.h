@@ -170,6 +170,18 @@ int sdm_remove_zero(sdm_t *h, int64_t *n_sd_out);
 int sdm_moments(sdm_t *h, int per_cell, int64_t *m0_dev, double *m1_dev, double *m2_dev);
 int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, double *m2_host);
 
+/* The spectrum product of Fig. 6: mass of droplets per unit of ln r [kg per m^3 of air per
+ * unit ln r] on n_bins bins (1 <= n_bins <= SDM_MAX_BINS), all cells together.  Bin b holds the droplets with
+ * v_edges_host[b] <= v < v_edges_host[b+1] (volumes, strictly increasing, n_bins + 1 values); its value is
+ * (sum xi*v) * rho / V / dlnr_host[b], where dlnr_host[b] = ln(r_{b+1} / r_b) > 0 is supplied by the caller
+ * (no logarithm is evaluated by the library), rho is the particle density [kg/m^3] and V the volume of air
+ * the state represents [m^3]; then n_smooth (>= 0; the paper: 2) passes of a centered five-bin running mean
+ * whose window is truncated at the ends (R17).  All array arguments are HOST pointers; out_host
+ * receives n_bins values.  SYNCHRONOUS.  The bin sums are fp64 sums in no fixed order (<= 1e-12 relative). */
+#define SDM_MAX_BINS 1024
+int sdm_spectrum(sdm_t *h, int32_t n_bins, const double *v_edges_host, const double *dlnr_host, double rho,
+                 double V, int32_t n_smooth, double *out_host);
+
 /* Exports the permutation and cell table of the LAST sdm_coalescence_step (parity / debugging;
  * the paper's `idx` and `cell_start`): idx_dev[n_sd] (storage indices in
  * cell-major, key-ascending order), cell_start_dev[n_cell + 1].  Either may be NULL.  The copies

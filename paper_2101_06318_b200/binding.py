@@ -34,7 +34,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
-    "sdm_set_efficiency_table",
+    "sdm_set_efficiency_table", "sdm_spectrum",
 )
 MAX_ATTR = 8
 
@@ -78,6 +78,7 @@ def load_library() -> C.CDLL:
     L.sdm_set_attributes.argtypes = [vp, vp, i64]
     L.sdm_get_attributes.argtypes = [vp, vp, i64]
     L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
+    L.sdm_spectrum.argtypes = [vp, i32, vp, vp, dbl, dbl, i32, vp]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
     L.sdm_set_state.argtypes = [vp, i64, vp, vp, vp]
@@ -189,6 +190,19 @@ class SDM:
         n = xi.shape[0]
         self._host(xi, t.int64), self._host(v, t.float64), self._host(cell_id, t.int32)
         self._check(self._lib.sdm_set_state_host(self._h, n, self._p(xi), self._p(v), self._p(cell_id)))
+
+    def spectrum(self, v_edges, dlnr, rho, V, n_smooth=2):
+        """Mass density per unit ln r on the bins v_edges (numpy float64 host arrays in, numpy array out)."""
+        import numpy as np
+
+        v_edges = np.ascontiguousarray(v_edges, dtype=np.float64)
+        dlnr = np.ascontiguousarray(dlnr, dtype=np.float64)
+        assert v_edges.shape[0] == dlnr.shape[0] + 1
+        out = np.zeros(dlnr.shape[0], dtype=np.float64)
+        self._check(self._lib.sdm_spectrum(self._h, int(dlnr.shape[0]), v_edges.ctypes.data_as(C.c_void_p),
+                                           dlnr.ctypes.data_as(C.c_void_p), float(rho), float(V), int(n_smooth),
+                                           out.ctypes.data_as(C.c_void_p)))
+        return out
 
     def set_efficiency_table(self, r_grid, E):
         """Collection efficiencies for KERNEL_GRAVITATIONAL_TABULATED: numpy float64 r_grid[n_r], E[n_r, n_r]."""

@@ -18,6 +18,7 @@
 #include "sdm_fused.cuh"
 #include "sdm_fused_count.cuh"
 #include "sdm_general.cuh"
+#include "sdm_spectrum.cuh"
 
 using namespace sdmk;
 
@@ -29,7 +30,7 @@ constexpr int kMinSegCap = 8;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t xi, v, attr, eff, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
+    size_t xi, v, attr, eff, spec, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
         bucket_cnt, tile_status, part0, part1, part2, mom_out, ctrl, total;
     int64_t nb_max, n_tiles, attr_stride;
 };
@@ -61,6 +62,7 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.part2 = take((size_t)kMomentBlocks * 8);
     L.mom_out = take(3 * 8);
     L.ctrl = take(sizeof(Ctrl));
+    L.spec = take((size_t)(4 * SDM_MAX_BINS + 1) * 8);          // spectrum: edges, widths, sums, result
     L.eff = take((size_t)(SDM_MAX_EFF_GRID + SDM_MAX_EFF_GRID * SDM_MAX_EFF_GRID) * 8);   // efficiency grid + table
     L.total = off;
     return L;
@@ -75,6 +77,7 @@ struct sdm {
     int32_t n_cell = 0;
     int32_t n_attr = 1;          // extensive attributes per droplet, volume included
     double *attr = nullptr;      // rows 1..n_attr-1
+    double *spec = nullptr;      // spectrum scratch: edges [SDM_MAX_BINS+1], dlnr, sums, out [SDM_MAX_BINS each]
     double *eff = nullptr;       // efficiency grid [SDM_MAX_EFF_GRID] followed by the table
     int eff_n = 0;               // 0: no table loaded
     double eff_max = 0.0;        // largest table entry (screening bounds)
@@ -405,7 +408,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
 
 extern "C" {
 
-int sdm_version(void) { return 1002; }
+int sdm_version(void) { return 1003; }
 
 size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
@@ -455,6 +458,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->v = reinterpret_cast<double *>(h->ws + L.v);
     h->attr = reinterpret_cast<double *>(h->ws + L.attr);
     h->eff = reinterpret_cast<double *>(h->ws + L.eff);
+    h->spec = reinterpret_cast<double *>(h->ws + L.spec);
     h->cell = reinterpret_cast<int32_t *>(h->ws + L.cell);
     h->idx = reinterpret_cast<int *>(h->ws + L.idx);
     h->order = reinterpret_cast<int *>(h->ws + L.order);
@@ -495,6 +499,8 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     }
     e = cudaMemsetAsync(h->ctrl, 0, sizeof(Ctrl), h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(ctrl)");
+    e = cudaMemsetAsync(h->spec, 0, (size_t)(4 * SDM_MAX_BINS + 1) * 8, h->stream);
+    if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(spec)");
     e = cudaMemsetAsync(h->cell_cnt, 0, ((size_t)n_cell + 1) * 4, h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(cell_cnt)");
     e = cudaMemsetAsync(h->bucket_cnt, 0, ((size_t)h->L.nb_max + 1) * 4, h->stream);
@@ -749,6 +755,31 @@ int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, 
     SDM_CUDA(h, cudaMemcpyAsync(m0_host, d0, (size_t)h->n_cell * 8, cudaMemcpyDeviceToHost, h->stream));
     SDM_CUDA(h, cudaMemcpyAsync(m1_host, d1, (size_t)h->n_cell * 8, cudaMemcpyDeviceToHost, h->stream));
     SDM_CUDA(h, cudaMemcpyAsync(m2_host, d2, (size_t)h->n_cell * 8, cudaMemcpyDeviceToHost, h->stream));
+    SDM_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SDM_OK;
+}
+
+int sdm_spectrum(sdm_t *h, int32_t n_bins, const double *v_edges_host, const double *dlnr_host, double rho,
+                 double V, int32_t n_smooth, double *out_host)
+{
+    if (!h) return SDM_EINVAL;
+    if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
+    if (n_bins < 1 || n_bins > SDM_MAX_BINS) return fail(h, SDM_EINVAL, "need 1 <= n_bins <= SDM_MAX_BINS");
+    if (!v_edges_host || !dlnr_host || !out_host) return fail(h, SDM_EINVAL, "spectrum pointer is NULL");
+    if (!(rho > 0.0) || !(V > 0.0) || !std::isfinite(rho) || !std::isfinite(V) || n_smooth < 0 || n_smooth > 64)
+        return fail(h, SDM_EINVAL, "need rho > 0, V > 0, 0 <= n_smooth <= 64");
+    for (int b = 0; b <= n_bins; ++b) {
+        if (!std::isfinite(v_edges_host[b]) || (b > 0 && !(v_edges_host[b] > v_edges_host[b - 1])))
+            return fail(h, SDM_EINVAL, "bin edges must be finite and strictly increasing");
+        if (b < n_bins && (!(dlnr_host[b] > 0.0) || !std::isfinite(dlnr_host[b])))
+            return fail(h, SDM_EINVAL, "bin widths must be finite and > 0");
+    }
+    double *edges = h->spec, *dlnr = edges + SDM_MAX_BINS + 1, *sums = dlnr + SDM_MAX_BINS, *out = sums + SDM_MAX_BINS;
+    SDM_CUDA(h, cudaMemcpyAsync(edges, v_edges_host, (size_t)(n_bins + 1) * 8, cudaMemcpyHostToDevice, h->stream));
+    SDM_CUDA(h, cudaMemcpyAsync(dlnr, dlnr_host, (size_t)n_bins * 8, cudaMemcpyHostToDevice, h->stream));
+    SDM_LAUNCH(h, k_spectrum_bin, grid_for(h, h->n_ub, 256, 4), 256, 0, h->xi, h->v, h->ctrl, n_bins, edges, sums);
+    SDM_LAUNCH(h, k_spectrum_finish, 1, kMaxBins, 0, n_bins, sums, dlnr, rho, V, n_smooth, out);
+    SDM_CUDA(h, cudaMemcpyAsync(out_host, out, (size_t)n_bins * 8, cudaMemcpyDeviceToHost, h->stream));
     SDM_CUDA(h, cudaStreamSynchronize(h->stream));
     return SDM_OK;
 }
