@@ -132,6 +132,14 @@ int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld);
 #define SDM_MAX_EFF_GRID 64
 int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host);
 
+/* Replaces the cell ids of the super-droplets currently in storage (cell_id_dev[n_sd], storage order) -- the
+ * hook for particle displacement, which the paper performs between coalescence steps and outside this API
+ * ("cell_id ... updated before this block"; "multi-dimensional" use).
+ * Multiplicities and attributes stay.  Validates 0 <= cell_id < n_cell and re-analyses the layout
+ * (cell-contiguous or not, largest cell), which decides the path of the next steps.  SYNCHRONOUS.  Errors:
+ * SDM_EINVAL (an id out of range: the state is then unusable), SDM_ESTATE. */
+int sdm_set_cell_id(sdm_t *h, const int32_t *cell_id_dev);
+
 /* Copies the current state out in storage order.  Any of the array pointers may be NULL.
  * SYNCHRONOUS (returns n_sd on the host).  The arrays must hold at least n_sd elements (capacity
  * is always enough). */

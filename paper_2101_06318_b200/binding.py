@@ -34,7 +34,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
-    "sdm_set_efficiency_table", "sdm_spectrum",
+    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id",
 )
 MAX_ATTR = 8
 
@@ -78,6 +78,7 @@ def load_library() -> C.CDLL:
     L.sdm_set_attributes.argtypes = [vp, vp, i64]
     L.sdm_get_attributes.argtypes = [vp, vp, i64]
     L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
+    L.sdm_set_cell_id.argtypes = [vp, vp]
     L.sdm_spectrum.argtypes = [vp, i32, vp, vp, dbl, dbl, i32, vp]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
@@ -213,6 +214,11 @@ class SDM:
         assert E.shape == (r_grid.shape[0], r_grid.shape[0])
         self._check(self._lib.sdm_set_efficiency_table(self._h, int(r_grid.shape[0]), r_grid.ctypes.data_as(C.c_void_p),
                                                        E.ctypes.data_as(C.c_void_p)))
+
+    def set_cell_id(self, cell_id):
+        """New cell ids (int32 device tensor, storage order, current n_sd entries) after displacement."""
+        self._dev(cell_id, self.torch.int32)
+        self._check(self._lib.sdm_set_cell_id(self._h, self._p(cell_id)))
 
     def set_attributes(self, attr):
         """Rows 1..n_attr-1 of the attribute block: a contiguous float64 device tensor [n_attr-1, n_sd]."""

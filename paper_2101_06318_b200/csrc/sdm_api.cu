@@ -408,7 +408,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
 
 extern "C" {
 
-int sdm_version(void) { return 1003; }
+int sdm_version(void) { return 1004; }
 
 size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
@@ -586,6 +586,36 @@ int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const dou
         SDM_CUDA(h, cudaMemcpyAsync(h->cell, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, h->stream));
     }
     return load_state_common(h, n_sd);
+}
+
+int sdm_set_cell_id(sdm_t *h, const int32_t *cell_id_dev)
+{
+    if (!h) return SDM_EINVAL;
+    if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
+    int rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    const int64_t n = h->ctrl_host->n;
+    h->n_ub = n;
+    if (n > 0 && !cell_id_dev) return fail(h, SDM_EINVAL, "cell id pointer is NULL");
+    h->stepped = false;
+    h->table_produced = false;
+    h->tables_ready = false;
+    if (n > 0) SDM_CUDA(h, cudaMemcpyAsync(h->cell, cell_id_dev, (size_t)n * 4, cudaMemcpyDeviceToDevice, h->stream));
+    // reset the layout fields of the control block (cell_cnt[] is all zero between calls)
+    SDM_CUDA(h, cudaMemsetAsync(&h->ctrl->unsorted, 0, sizeof(int), h->stream));
+    SDM_CUDA(h, cudaMemsetAsync(&h->ctrl->max_count, 0, sizeof(int), h->stream));
+    if (n > 0)
+        SDM_LAUNCH(h, k_analyze_cells, grid_for(h, n, 256, 16), 256, 0, h->cell, (int)n, h->n_cell, h->cell_cnt, h->ctrl);
+    SDM_LAUNCH(h, k_max_count, grid_for(h, h->n_cell, 256, 8), 256, 0, h->cell_cnt, h->n_cell, h->ctrl);
+    rc = read_ctrl(h);
+    if (rc != SDM_OK) return rc;
+    if (h->ctrl_host->invalid) {
+        h->valid = false;
+        return fail(h, SDM_EINVAL, "cell id validation failed: need 0 <= cell_id < n_cell");
+    }
+    h->max_count = h->ctrl_host->max_count;
+    h->sorted = (h->ctrl_host->unsorted == 0);
+    return SDM_OK;
 }
 
 int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host)

@@ -71,6 +71,30 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
     }
 }
 
+// sdm_set_cell_id (NEXT-4): new cell ids for the droplets in storage -- range check, sortedness, counts
+__global__ void k_analyze_cells(const int32_t *__restrict__ cell, int n, int n_cell, int *__restrict__ cell_cnt,
+                                Ctrl *ctrl)
+{
+    int bad = 0, unsorted = 0;
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane_id();
+        int c = -1;
+        if (i < n) {
+            c = cell[i];
+            if (c < 0 || c >= n_cell) { bad = 1; c = -1; }
+            else if (i > 0 && cell[i - 1] > c) unsorted = 1;
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
+        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(&cell_cnt[c], __popc(peers));
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    unsorted = __any_sync(0xffffffffu, unsorted);
+    if (lane_id() == 0) {
+        if (bad) atomicOr(&ctrl->invalid, 1);
+        if (unsorted) atomicOr(&ctrl->unsorted, 1);
+    }
+}
+
 // sdm_set_attributes: every value of the extra attribute rows must be finite
 __global__ void k_check_attr(const AttrView av, int n, Ctrl *ctrl)
 {
