@@ -1,7 +1,8 @@
-// sdm_general.cuh -- general path (any storage order, cells of any size): the per-segment sort.
+// sdm_general.cuh -- general path (any storage order, cells of any size): counting sort by cell / key
+// bucket, per-segment sort, pairs.
 //
 // A "segment" is a cell, or -- for cells larger than the warp capacity -- the droplets of a cell whose
-// sort key has the same top B bits (sdm_kernels.cuh: split_bits, k_bucket_count, k_scatter).  order[]
+// sort key has the same top B bits (split_bits in sdm_kernels.cuh; k_gen_count, k_gen_scatter below).  order[]
 // lists the storage indices of every segment contiguously; this kernel puts each segment into
 // (key64, storage index) order (row a3; R6-R7) and writes idx.
 //
