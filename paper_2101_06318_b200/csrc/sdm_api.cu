@@ -31,7 +31,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xi, v, attr, eff, spec, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
-        bucket_cnt, tile_status, part0, part1, part2, mom_out, ctrl, total;
+        bucket_cnt, tile_status, scan_status, part0, part1, part2, mom_out, ctrl, total;
     int64_t nb_max, n_tiles, attr_stride;
 };
 
@@ -57,6 +57,7 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.bucket_start = take(((size_t)L.nb_max + 1) * 4);
     L.bucket_cnt = take(((size_t)L.nb_max + 1) * 4);
     L.tile_status = take((size_t)L.n_tiles * 8);
+    L.scan_status = take((size_t)(((int64_t)n_cell + L.nb_max) / 2048 + 4) * 8);
     L.part0 = take((size_t)kMomentBlocks * 8);
     L.part1 = take((size_t)kMomentBlocks * 8);
     L.part2 = take((size_t)kMomentBlocks * 8);
@@ -90,7 +91,7 @@ struct sdm {
     int32_t *cell = nullptr;
     int *idx = nullptr, *order = nullptr, *cell_start = nullptr, *cell_start2 = nullptr, *cell_cnt = nullptr,
         *cell_bits = nullptr, *bucket_base = nullptr, *bucket_start = nullptr, *bucket_cnt = nullptr;
-    unsigned long long *tile_status = nullptr;
+    unsigned long long *tile_status = nullptr, *scan_status = nullptr;
     int64_t *part0 = nullptr;
     double *part1 = nullptr, *part2 = nullptr;
     int64_t *mom0 = nullptr;
@@ -333,15 +334,23 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     const int n_seg = split ? h->n_seg : h->n_cell;
     int *seg_start = split ? h->bucket_start : h->cell_start;
     const int g = grid_for(h, n_ub, 256, 16);
-    SDM_LAUNCH(h, k_gen_count, h->n_cell <= kCellCountBins ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell, h->ctrl,
-               h->n_cell, split, h->cell_bits, h->bucket_base, h->cell_cnt, h->bucket_cnt, prm);
-    SDM_LAUNCH(h, k_gen_scan, 1, kScanThreads, 0, h->cell_cnt, h->n_cell, h->cell_start, split, h->bucket_cnt,
-               n_seg, h->bucket_start);
+    // idx[] carries the arrival ranks from the count to the scatter pass; the sort kernel overwrites it afterwards
+    SDM_LAUNCH(h, k_gen_count, (split && h->n_cell <= kCellCountBins) ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell,
+               h->ctrl, h->n_cell, split, h->cell_bits, h->bucket_base, h->cell_cnt, h->bucket_cnt, h->idx, prm);
+    const int scan_tiles = (h->n_cell + kScanTile - 1) / kScanTile + (split ? (n_seg + kScanTile - 1) / kScanTile : 0);
+    SDM_LAUNCH(h, k_gen_scan, scan_tiles < 4 * h->num_sms ? scan_tiles : 4 * h->num_sms, kScanTileThreads, 0, h->cell_cnt,
+               h->n_cell, h->cell_start, split, h->bucket_cnt, n_seg, h->bucket_start, h->ctrl, h->scan_status);
     SDM_LAUNCH(h, k_gen_scatter, g, 256, 0, h->cell, h->ctrl, split, h->cell_bits, h->bucket_base, seg_start,
-               h->bucket_cnt, h->order, prm);
-    SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
-                            kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
-                            h->cell, h->cell_bits, h->cell_start, h->bucket_cnt, h->idx, h->xi, h->v, h->ctrl, prm));
+               h->idx, h->order, prm);
+    // four droplets per lane when no segment can exceed 128 (half the Philox blocks per warp), else eight
+    if ((split ? general_cap(h) : h->max_count) <= 128)
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<4>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
+                                kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
+                                h->cell, h->cell_bits, h->cell_start, h->idx, h->xi, h->v, h->ctrl, prm));
+    else
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<8>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
+                                kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
+                                h->cell, h->cell_bits, h->cell_start, h->idx, h->xi, h->v, h->ctrl, prm));
     if (split)
         SDM_LAUNCH(h, k_pairs_straddle, grid_for(h, n_seg, 256, 8), 256, 0, seg_start, n_seg, h->idx, h->cell,
                    h->cell_start, h->xi, h->v, h->ctrl, prm);
@@ -361,7 +370,10 @@ int enqueue_remove_zero(sdm_t *h)
 int enqueue_moments(sdm_t *h, int per_cell, int64_t *m0, double *m1, double *m2)
 {
     if (!per_cell) {
-        SDM_LAUNCH(h, k_moments_global, kMomentBlocks, kMomentThreads, 0, h->xi, h->v, h->ctrl, h->part0,
+        // small states: fewer CTAs (the last CTA sums one partial per CTA)
+        int64_t mb = (h->n_ub / 2 + (int64_t)kMomentThreads * 4 - 1) / ((int64_t)kMomentThreads * 4);
+        mb = mb < 1 ? 1 : (mb > kMomentBlocks ? kMomentBlocks : mb);
+        SDM_LAUNCH(h, k_moments_global, (int)mb, kMomentThreads, 0, h->xi, h->v, h->ctrl, h->part0,
                    h->part1, h->part2, m0, m1, m2);
         return SDM_OK;
     }
@@ -377,7 +389,9 @@ int load_state_common(sdm_t *h, int64_t n_sd)
     Ctrl zero{};
     zero.n = (int)n_sd;
     zero.epoch = 1;                                   // tile status words are tagged; 0 = never written
+    zero.scan_epoch = 1;
     SDM_CUDA(h, cudaMemsetAsync(h->tile_status, 0, (size_t)h->L.n_tiles * 8, h->stream));
+    SDM_CUDA(h, cudaMemsetAsync(h->scan_status, 0, (size_t)(((int64_t)h->n_cell + h->L.nb_max) / 2048 + 4) * 8, h->stream));
     if (h->n_attr > 1)
         SDM_CUDA(h, cudaMemsetAsync(h->attr, 0, (size_t)(h->n_attr - 1) * (size_t)h->L.attr_stride * 8, h->stream));
     SDM_CUDA(h, cudaMemcpyAsync(h->ctrl, &zero, sizeof(Ctrl), cudaMemcpyHostToDevice, h->stream));
@@ -470,6 +484,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->bucket_start = reinterpret_cast<int *>(h->ws + L.bucket_start);
     h->bucket_cnt = reinterpret_cast<int *>(h->ws + L.bucket_cnt);
     h->tile_status = reinterpret_cast<unsigned long long *>(h->ws + L.tile_status);
+    h->scan_status = reinterpret_cast<unsigned long long *>(h->ws + L.scan_status);
     h->part0 = reinterpret_cast<int64_t *>(h->ws + L.part0);
     h->part1 = reinterpret_cast<double *>(h->ws + L.part1);
     h->part2 = reinterpret_cast<double *>(h->ws + L.part2);
@@ -485,7 +500,8 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     };
     e = cudaMallocHost(reinterpret_cast<void **>(&h->ctrl_host), sizeof(Ctrl));
     if (e != cudaSuccess) { h->ctrl_host = nullptr; return bail(e, "cudaMallocHost"); }
-    e = cudaFuncSetAttribute(k_segment_sort_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
+    e = cudaFuncSetAttribute(k_segment_sort_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_segment_sort_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_pairs)");
     e = cudaFuncSetAttribute(k_fused_cells_count<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);

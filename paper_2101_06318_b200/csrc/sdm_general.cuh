@@ -38,10 +38,13 @@ constexpr size_t kGenSmemBytes = kGenWarps * sizeof(GenSmem);
 
 // Sort words of one segment: x[k] belongs to local droplet k*32+lane on entry (id[k] its storage index),
 // and to sorted position 8*lane+k on return.  shift = key bits shared by the whole segment.
-__device__ __forceinline__ void count_sort_ids(const int (&id)[8], int m, int lane, int shift, uint64_t step,
-                                               const PhiloxKey &rk, GenSmem *sm, uint32_t sm_base, uint32_t (&x)[8])
+// E = 8 (segments up to 256) or 4 (up to 128: half the Philox blocks and sort words per warp).
+template <int E>
+__device__ __forceinline__ void count_sort_ids(const int (&id)[E], int m, int lane, int shift, uint64_t step,
+                                               const PhiloxKey &rk, GenSmem *sm, uint32_t sm_base, uint32_t (&x)[E])
 {
-    constexpr int E = 8, L = 32, N = kGenCap;
+    constexpr int L = 32, N = L * E;
+    static_assert(E == 4 || E == 8, "rows per lane");
     const int nrem = m - lane;
     uint32_t old[E];
 #pragma unroll
@@ -87,21 +90,22 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[8], int m, int la
         }
     }
     __syncwarp();
-    {
-        const uint4 q0 = reinterpret_cast<const uint4 *>(sm->slot)[2 * lane];
-        const uint4 q1 = reinterpret_cast<const uint4 *>(sm->slot)[2 * lane + 1];
-        x[0] = q0.x; x[1] = q0.y; x[2] = q0.z; x[3] = q0.w;
-        x[4] = q1.x; x[5] = q1.y; x[6] = q1.z; x[7] = q1.w;
+#pragma unroll
+    for (int q = 0; q < E / 4; ++q) {
+        const uint4 w = reinterpret_cast<const uint4 *>(sm->slot)[(E / 4) * lane + q];
+        x[4 * q] = w.x; x[4 * q + 1] = w.y; x[4 * q + 2] = w.z; x[4 * q + 3] = w.w;
     }
     for (uint32_t r = 0; r < rounds; r += 2) {
-        cex(x[0], x[1]); cex(x[2], x[3]); cex(x[4], x[5]); cex(x[6], x[7]);
+#pragma unroll
+        for (int k = 0; k + 1 < E; k += 2) cex(x[k], x[k + 1]);
         uint32_t nx0 = __shfl_down_sync(0xffffffffu, x[0], 1);
-        uint32_t px7 = __shfl_up_sync(0xffffffffu, x[7], 1);
+        uint32_t pxl = __shfl_up_sync(0xffffffffu, x[E - 1], 1);
         if (lane == 31) nx0 = 0xFFFFFFFFu;
-        if (lane == 0) px7 = 0u;
-        cex(x[1], x[2]); cex(x[3], x[4]); cex(x[5], x[6]);
-        x[7] = min(x[7], nx0);
-        x[0] = max(x[0], px7);
+        if (lane == 0) pxl = 0u;
+#pragma unroll
+        for (int k = 1; k + 1 < E; k += 2) cex(x[k], x[k + 1]);
+        x[E - 1] = min(x[E - 1], nx0);
+        x[0] = max(x[0], pxl);
     }
 }
 
@@ -112,7 +116,7 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[8], int m, int la
 // The split of large cells (cell_bits[c] = B key bits, bucket_base[c] = first segment of cell c) is
 // decided ONCE per loaded state from the cell counts (k_cell_scan with split = 1): cells never grow
 // (PAPER.md:9, 77), so the segments only get smaller afterwards, and idx does not depend on B.
-// Invariant between steps: cell_cnt[] and seg_cnt[] are all zero (every consumer clears what it read).
+// Invariant between steps: cell_cnt[] and seg_cnt[] are all zero (the scan clears what it read).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int segment_of(int c, uint32_t key_hi, const int *__restrict__ cell_bits,
                                           const int *__restrict__ bucket_base)
@@ -121,28 +125,47 @@ __device__ __forceinline__ int segment_of(int c, uint32_t key_hi, const int *__r
     return bucket_base[c] + (B > 0 ? (int)(key_hi >> (32 - B)) : 0);
 }
 
-// Row a2: per-cell counts (warp-aggregated; CTA-privatised when there are few cells) and, when cells
-// are split, per-segment counts (needs the droplet's Philox block, row a1).
+// Row a2: per-cell counts and, when cells are split, per-segment counts (needs the droplet's Philox block,
+// row a1).  The counting atomic that a droplet's segment receives also RETURNS the droplet's arrival rank in
+// that segment (rank[i]), so the scatter pass needs no atomics of its own.  Lanes of a warp that hit the same
+// counter send one atomic (a box is ONE cell: same-address atomics would serialise in L2); cell counters that
+// are not needed for ranks (split mode) are CTA-privatised in shared memory when there are few cells.
 __global__ void __launch_bounds__(256)
 k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell, int split,
             const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
-            int *__restrict__ cell_cnt, int *__restrict__ seg_cnt, const __grid_constant__ StepParams prm)
+            int *__restrict__ cell_cnt, int *__restrict__ seg_cnt, int *__restrict__ rank,
+            const __grid_constant__ StepParams prm)
 {
     __shared__ int s_cnt[kCellCountBins];
     const int n = ctrl->n;
-    const bool priv = n_cell <= kCellCountBins;
+    const int lane = lane_id();
+    const bool priv = split && n_cell <= kCellCountBins;
     if (priv) {
         for (int c = threadIdx.x; c < n_cell; c += blockDim.x) s_cnt[c] = 0;
         __syncthreads();
     }
     for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
-        const int i = i0 + lane_id();
+        const int i = i0 + lane;
         const int c = (i < n) ? cell[i] : -1;
         const unsigned peers = __match_any_sync(0xffffffffu, c);
-        if (c >= 0 && (int)(__ffs(peers) - 1) == lane_id()) atomicAdd(priv ? &s_cnt[c] : &cell_cnt[c], __popc(peers));
-        if (split && c >= 0) {
-            const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
-            atomicAdd(&seg_cnt[segment_of(c, w.y, cell_bits, bucket_base)], 1);
+        const bool leader = (int)(__ffs(peers) - 1) == lane;
+        if (!split) {                                   // segment == cell: the cell counter gives the rank
+            int base = 0;
+            if (c >= 0 && leader) base = atomicAdd(&cell_cnt[c], __popc(peers));
+            base = __shfl_sync(0xffffffffu, base, __ffs(peers) - 1);
+            if (c >= 0) rank[i] = base + __popc(peers & ((1u << lane) - 1u));
+        } else {
+            if (c >= 0 && leader) atomicAdd(priv ? &s_cnt[c] : &cell_cnt[c], __popc(peers));
+            int seg = -1;
+            if (c >= 0) {
+                const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
+                seg = segment_of(c, w.y, cell_bits, bucket_base);
+            }
+            const unsigned speers = __match_any_sync(0xffffffffu, seg);
+            int base = 0;
+            if (seg >= 0 && (int)(__ffs(speers) - 1) == lane) base = atomicAdd(&seg_cnt[seg], __popc(speers));
+            base = __shfl_sync(0xffffffffu, base, __ffs(speers) - 1);
+            if (seg >= 0) rank[i] = base + __popc(speers & ((1u << lane) - 1u));
         }
     }
     if (priv) {
@@ -153,47 +176,121 @@ k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int
 }
 
 // Exclusive scans: cell counts -> cell_start[n_cell+1] and (split) segment counts -> seg_start[n_seg+1].
-// Clears the counters it reads.  One CTA.
-__global__ void __launch_bounds__(kScanThreads)
+// Clears the counters it reads.  Tiles of 2048 counters, coalesced loads and stores through shared memory,
+// chained by decoupled look-back (tiles handed out in order by a ticket, epoch-tagged status words as in
+// k_compact); the two tables are two independent chains of one launch.  A single-CTA scan took 13-22 us for
+// 16 K counters (one SM's load/store path); this one is at the launch floor.
+constexpr int kScanTile = 2048;
+constexpr int kScanTileThreads = 256;
+
+__global__ void __launch_bounds__(kScanTileThreads)
 k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start, int split,
-           int *__restrict__ seg_cnt, int n_seg, int *__restrict__ seg_start)
+           int *__restrict__ seg_cnt, int n_seg, int *__restrict__ seg_start, Ctrl *ctrl,
+           unsigned long long *__restrict__ status)
 {
-    __shared__ int s_warp[33];
-    for (int pass = 0; pass < (split ? 2 : 1); ++pass) {
-        int *cnt = pass ? seg_cnt : cell_cnt;
-        int *start = pass ? seg_start : cell_start;
-        const int m = pass ? n_seg : n_cell;
-        int carry = 0;
-        for (int base = 0; base < m; base += kScanThreads * kScanItems) {
-            const int c0 = base + threadIdx.x * kScanItems;
-            int loc[kScanItems];
-            int sum = 0;
-#pragma unroll
-            for (int k = 0; k < kScanItems; ++k) {
-                loc[k] = (c0 + k < m) ? cnt[c0 + k] : 0;
-                sum += loc[k];
-            }
-            int total;
-            int run = carry + block_exclusive_scan(sum, s_warp, total);
-#pragma unroll
-            for (int k = 0; k < kScanItems; ++k) {
-                if (c0 + k < m) { start[c0 + k] = run; cnt[c0 + k] = 0; }
-                run += loc[k];
-            }
-            carry += total;
-            __syncthreads();
-        }
-        if (threadIdx.x == 0) start[m] = carry;
+    constexpr int kItems = kScanTile / kScanTileThreads;          // 8
+    __shared__ int s_val[kScanTile + kScanTile / 32];             // padded: index e + e/32
+    __shared__ int s_warp[kScanTileThreads / 32];
+    __shared__ int s_tile, s_prefix;
+    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
+    const int tiles_a = (n_cell + kScanTile - 1) / kScanTile;
+    const int tiles_b = split ? (n_seg + kScanTile - 1) / kScanTile : 0;
+    const unsigned long long tag = (unsigned long long)(ctrl->scan_epoch & 0x3fffffffu) << 34;
+    while (true) {
         __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&ctrl->scan_ticket, 1);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= tiles_a + tiles_b) break;
+        const bool second = tile >= tiles_a;
+        int *cnt = second ? seg_cnt : cell_cnt;
+        int *start = second ? seg_start : cell_start;
+        const int m = second ? n_seg : n_cell;
+        const int chain0 = second ? tiles_a : 0;                  // first tile of this chain
+        const int base = (tile - chain0) * kScanTile;
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int e = k * kScanTileThreads + tid;
+            s_val[e + (e >> 5)] = (base + e < m) ? cnt[base + e] : 0;
+        }
+        __syncthreads();
+        int loc[kItems], sum = 0;
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int e = tid * kItems + k;
+            loc[k] = s_val[e + (e >> 5)];
+            sum += loc[k];
+        }
+        int inc = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += t;
+        }
+        if (lane == 31) s_warp[warp] = inc;
+        __syncthreads();
+        int woff = 0, tile_total = 0;
+#pragma unroll
+        for (int w = 0; w < kScanTileThreads / 32; ++w) {
+            const int cw = s_warp[w];
+            if (w < warp) woff += cw;
+            tile_total += cw;
+        }
+        if (tid == 0) {
+            int excl = 0;
+            volatile unsigned long long *vs = status;
+            __threadfence();
+            if (tile == chain0) {
+                vs[tile] = tag | kFlagInclusive | (unsigned long long)(unsigned int)tile_total;
+            } else {
+                vs[tile] = tag | kFlagAggregate | (unsigned long long)(unsigned int)tile_total;
+                int t = tile - 1;
+                while (true) {
+                    const unsigned long long st = vs[t];
+                    if ((st >> 34) != (tag >> 34) || ((st >> 32) & 3ull) == 0) continue;   // not published yet
+                    excl += (int)(st & 0xffffffffull);
+                    if (((st >> 32) & 3ull) == 2) break;
+                    --t;
+                }
+                vs[tile] = tag | kFlagInclusive | (unsigned long long)(unsigned int)(excl + tile_total);
+            }
+            __threadfence();
+            s_prefix = excl;
+        }
+        __syncthreads();
+        int run = s_prefix + woff + inc - sum;
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int e = tid * kItems + k;
+            s_val[e + (e >> 5)] = run;
+            run += loc[k];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int e = k * kScanTileThreads + tid;
+            if (base + e < m) { start[base + e] = s_val[e + (e >> 5)]; cnt[base + e] = 0; }
+        }
+        if (tid == 0 && base + kScanTile >= m) start[m] = s_prefix + tile_total;      // the chain's last tile
+    }
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(&ctrl->scan_done, 1u) == gridDim.x - 1) {
+            __threadfence();
+            ctrl->scan_ticket = 0;
+            ctrl->scan_done = 0;
+            ctrl->scan_epoch = ctrl->scan_epoch + 1u;
+        }
     }
 }
 
-// order[] = storage indices grouped by segment (arbitrary order inside; the sort makes it unique).
-// cursor[] must be zero on entry; the sort kernel clears it again.
+// order[] = storage indices grouped by segment, at the arrival rank k_gen_count handed out (any order inside a
+// segment would do; the sort makes it unique).
 __global__ void __launch_bounds__(256)
 k_gen_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int split,
               const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
-              const int *__restrict__ seg_start, int *__restrict__ cursor, int *__restrict__ order,
+              const int *__restrict__ seg_start, const int *__restrict__ rank, int *__restrict__ order,
               const __grid_constant__ StepParams prm)
 {
     const int n = ctrl->n;
@@ -204,8 +301,7 @@ k_gen_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, i
             const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
             b = segment_of(c, w.y, cell_bits, bucket_base);
         }
-        const int pos = atomicAdd(&cursor[b], 1);
-        order[seg_start[b] + pos] = i;
+        order[seg_start[b] + rank[i]] = i;
     }
 }
 
@@ -230,15 +326,16 @@ __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, in
 
 // seg_start[0..n_seg]: segment boundaries in order[]; split != 0: segments are pieces of cells and
 // cell_bits[cell] gives the key bits a segment's droplets share.  seg_cap <= 256: larger segments are
-// ranked by counting (tests lower it).  Clears cursor[seg].
+// ranked by counting (tests lower it).
+template <int E>
 __global__ void __launch_bounds__(kGenWarps * 32)
 k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, int seg_cap,
                      const int *__restrict__ order, const int32_t *__restrict__ cell,
                      const int *__restrict__ cell_bits, const int *__restrict__ cell_start,
-                     int *__restrict__ cursor, int *__restrict__ idx, int64_t *__restrict__ xi,
+                     int *__restrict__ idx, int64_t *__restrict__ xi,
                      double *__restrict__ v, Ctrl *ctrl, const __grid_constant__ StepParams prm)
 {
-    constexpr int E = 8, L = 32, N = kGenCap;
+    constexpr int L = 32, N = L * E;                      // segment capacity of this instantiation
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     GenSmem *sm = reinterpret_cast<GenSmem *>(smem_dyn) + (threadIdx.x >> 5);
     const int lane = lane_id();
@@ -247,13 +344,13 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
     const PhiloxKey &rk = prm.rk;
     for (int i = lane; i < 256; i += 32) sm->cnt[i] = 0;
     __syncwarp();
+    seg_cap = min(seg_cap, N);
     int packed_sum_ev = 0, packed_sum_z = 0, packed_sum_ex = 0;
     const int warps_total = gridDim.x * kGenWarps;
     for (int seg = blockIdx.x * kGenWarps + (threadIdx.x >> 5); seg < n_seg; seg += warps_total) {
         const int s = seg_start[seg];
         const int m = seg_start[seg + 1] - s;
         if (m == 0) continue;
-        if (lane == 0) cursor[seg] = 0;
         const int id0 = order[s];
         const int c = cell[id0];
         const int cs = cell_start[c], n_s = cell_start[c + 1] - cs;
@@ -276,7 +373,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
             }
             const int shift = split ? cell_bits[c] : 0;
             uint32_t x[E];
-            count_sort_ids(id, m, lane, shift, prm.step, rk, sm, sm_base, x);
+            count_sort_ids<E>(id, m, lane, shift, prm.step, rk, sm, sm_base, x);
             // adjacent words that share the truncated key differ by less than N
             const uint32_t nx0 = __shfl_down_sync(0xffffffffu, x[0], 1);
             uint32_t dmin = 0xFFFFFFFFu;

@@ -32,6 +32,10 @@ struct Ctrl {
     int pad0[1];
     unsigned long long n_events;   // pairs with gamma_tilde > 0
     unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
+    int scan_ticket;               // general path scan: tile ticket
+    unsigned int scan_done;        // general path scan: CTAs that have left the kernel
+    unsigned int scan_epoch;       // general path scan: tag of valid status words
+    int pad1;
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
