@@ -307,16 +307,17 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         if (h->lanes_per_cell == 16 && h->max_count > 128 && h->max_count <= 256) { E = 16; L = 16; }
         const int64_t warps_needed = ((int64_t)h->n_cell * L + 31) / 32;
         const int gf = grid_for(h, warps_needed * 32, kFusedWarps * 32, 8);
+#define SDM_FUSED_T(EE, LL, MM, TT)                                                                          \
+    SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, MM, TT>), gf, kFusedWarps * 32, 0, h->xi, h->v,            \
+                            h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1, h->part2, m0,    \
+                            m1, m2))
 #define SDM_FUSED(EE, LL)                                                                                    \
     do {                                                                                                     \
-        if (m0)                                                                                              \
-            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, true>), gf, kFusedWarps * 32, 0, h->xi, h->v,   \
-                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,       \
-                                    h->part2, m0, m1, m2));                                                  \
-        else                                                                                                 \
-            SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, false>), gf, kFusedWarps * 32, 0, h->xi, h->v,  \
-                                    h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1,       \
-                                    h->part2, m0, m1, m2));                                                  \
+        const bool tab_ = prm.kernel == SDM_KERNEL_GRAVITATIONAL_TABULATED;                                  \
+        if (m0 && tab_) SDM_FUSED_T(EE, LL, true, true);                                                     \
+        else if (m0) SDM_FUSED_T(EE, LL, true, false);                                                       \
+        else if (tab_) SDM_FUSED_T(EE, LL, false, true);                                                     \
+        else SDM_FUSED_T(EE, LL, false, false);                                                              \
     } while (0)
         if (E == 8 && L == 8) SDM_FUSED(8, 8);
         else if (E == 8 && L == 16) SDM_FUSED(8, 16);
@@ -324,6 +325,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         else if (E == 16 && L == 16) SDM_FUSED(16, 16);
         else SDM_FUSED(16, 32);
 #undef SDM_FUSED
+#undef SDM_FUSED_T
         return SDM_OK;
     }
     if (!h->tables_ready) {
@@ -335,7 +337,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     int *seg_start = split ? h->bucket_start : h->cell_start;
     const int g = grid_for(h, n_ub, 256, 16);
     // idx[] carries the arrival ranks from the count to the scatter pass; the sort kernel overwrites it afterwards
-    SDM_LAUNCH(h, k_gen_count, (split && h->n_cell <= kCellCountBins) ? grid_for(h, n_ub, 256, 4) : g, 256, 0, h->cell,
+    SDM_LAUNCH(h, k_gen_count, (split && h->n_cell <= kCellCountBins) ? grid_for(h, n_ub, 256, 8) : g, 256, 0, h->cell,
                h->ctrl, h->n_cell, split, h->cell_bits, h->bucket_base, h->cell_cnt, h->bucket_cnt, h->idx, prm);
     const int scan_tiles = (h->n_cell + kScanTile - 1) / kScanTile + (split ? (n_seg + kScanTile - 1) / kScanTile : 0);
     SDM_LAUNCH(h, k_gen_scan, scan_tiles < 4 * h->num_sms ? scan_tiles : 4 * h->num_sms, kScanTileThreads, 0, h->cell_cnt,

@@ -197,21 +197,25 @@ __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, doub
                                                   int32_t ktype, double kparam, const AttrView &av)
 {
     int64_t xa = xi[a], xb = xi[b];
+    double vj = v[a], vk = v[b];                         // four independent loads, one round trip
     int j = a, k = b;
     int64_t xj = xa, xk = xb;
-    if (xa < xb) { j = b; k = a; xj = xb; xk = xa; }     // PAPER.md:257-259 (strict <, R8)
+    if (xa < xb) {                                       // PAPER.md:257-259 (strict <, R8)
+        j = b; k = a; xj = xb; xk = xa;
+        const double t = vj; vj = vk; vk = t;
+    }
     if (xk == 0) return 0;                               // R11
-    double vj = v[j], vk = v[k];
     double K = (TAB && ktype == 2) ? coalescence_kernel_tabulated(kparam, vj, vk, av)
                                    : coalescence_kernel(ktype, kparam, vj, vk);
     double p = __dmul_rn(__dmul_rn(K, __ll2double_rn(xj)), norm);      // Eq. 3 in routine order (R3)
     double fl = floor(p);
+    double gamma = (u < __dsub_rn(p, fl)) ? __dadd_rn(fl, 1.0) : fl;       // PAPER.md:102, R4
+    if (gamma == 0.0) return 0;                          // gamma_tilde = min(0, q) = 0: the usual case, no division
     int64_t q = xj / xk;
     int64_t g;
     if (fl >= __ll2double_rn(q)) {
         g = q;                                           // cap reached without converting p (R8)
     } else {
-        double gamma = (u < __dsub_rn(p, fl)) ? __dadd_rn(fl, 1.0) : fl;   // PAPER.md:102, R4
         int64_t gi = __double2ll_rz(gamma);
         g = gi < q ? gi : q;                             // Eq. 4
     }

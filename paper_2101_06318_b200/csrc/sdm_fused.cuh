@@ -250,7 +250,7 @@ struct FusedTraits {
 
 // MOM: also produce the global moments (M0, M1, M2) of the state AFTER the step: the pre-step sums
 // are taken from the values streamed for the screening, and every event adds its exact change.
-template <int E, int L, bool MOM>
+template <int E, int L, bool MOM, bool TAB>
 __global__ void __launch_bounds__(kFusedWarps * 32, FusedTraits<E>::kMinBlocks)
 k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__restrict__ cell_start,
               int n_cell, int *__restrict__ idx, Ctrl *ctrl, StepParams prm, int64_t *__restrict__ part0,
@@ -283,7 +283,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             for (int gg = 0; gg < G; ++gg) {
                 const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
                 if (n2 <= N) continue;
-                const int pk = oversize_cell<true>(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
+                const int pk = oversize_cell<TAB>(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
                                              prm.seed, prm.step, my_delta, prm.attr);
                 events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
                 if (MOM) {
@@ -397,7 +397,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
 #pragma unroll
             for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
             __syncwarp();
-            const int pk = collide_flagged<true>(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
+            const int pk = collide_flagged<TAB>(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
                                            prm.kernel, prm.kparam, prm.seed, prm.step, my_delta, prm.attr);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
             if (MOM) {

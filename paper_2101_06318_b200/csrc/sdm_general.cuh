@@ -352,7 +352,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
         const int m = seg_start[seg + 1] - s;
         if (m == 0) continue;
         const int id0 = order[s];
-        const int c = cell[id0];
+        const int c = split ? cell[id0] : seg;            // unsplit: a segment is a cell
         const int cs = cell_start[c], n_s = cell_start[c + 1] - cs;
         int pk;
         if (m > seg_cap) {
