@@ -346,11 +346,11 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                h->idx, h->order, prm);
     // four droplets per lane when no segment can exceed 128 (half the Philox blocks per warp), else eight
     if ((split ? general_cap(h) : h->max_count) <= 128)
-        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<4>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<4>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 4),
                                 kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
                                 h->cell, h->cell_bits, h->cell_start, h->idx, h->xi, h->v, h->ctrl, prm));
     else
-        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<8>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 3),
+        SDM_TIMED(h, SDM_LAUNCH(h, k_segment_sort_pairs<8>, grid_for(h, (int64_t)n_seg * 32, kGenWarps * 32, 4),
                                 kGenWarps * 32, kGenSmemBytes, seg_start, n_seg, split, general_cap(h), h->order,
                                 h->cell, h->cell_bits, h->cell_start, h->idx, h->xi, h->v, h->ctrl, prm));
     if (split)

@@ -28,8 +28,9 @@ struct __align__(1024) GenSmem {
     uint32_t start[256];                  // shared-space byte address of each bin's first slot
     uint32_t slot[kGenCap];               // words grouped by bin
     int ids[kGenCap];                     // storage index of local droplet e
-    uint64_t key[kGenCap];                // exact path: full keys
-    int sid[kGenCap];                     // exact path: indices carried through the network
+    int sid[kGenCap];                     // sorted storage indices (input of the pair loop)
+    // exact path (truncated words tie): the full 64-bit keys reuse start[] and slot[], which are dead by then
+    __device__ uint64_t *key() { return reinterpret_cast<uint64_t *>(start); }
 };
 static_assert(sizeof(GenSmem) % 1024 == 0, "GenSmem must tile shared memory in 1 KB units");
 static_assert(offsetof(GenSmem, start) == 1024 && offsetof(GenSmem, slot) == 2048, "layout used by the address arithmetic");
@@ -328,7 +329,7 @@ __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, in
 // cell_bits[cell] gives the key bits a segment's droplets share.  seg_cap <= 256: larger segments are
 // ranked by counting (tests lower it).
 template <int E>
-__global__ void __launch_bounds__(kGenWarps * 32)
+__global__ void __launch_bounds__(kGenWarps * 32, 4)      // latency-bound gathers: occupancy over registers
 k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, int seg_cap,
                      const int *__restrict__ order, const int32_t *__restrict__ cell,
                      const int *__restrict__ cell_bits, const int *__restrict__ cell_start,
@@ -389,15 +390,15 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
                 for (int e = lane; e < P; e += 32) {
                     if (e < m) {
                         const int d = sm->ids[e];
-                        sm->key[e] = block_key64(droplet_block((uint32_t)d, prm.step, rk));
+                        sm->key()[e] = block_key64(droplet_block((uint32_t)d, prm.step, rk));
                         sm->sid[e] = d;
                     } else {
-                        sm->key[e] = ~0ull;
+                        sm->key()[e] = ~0ull;
                         sm->sid[e] = 0x7fffffff;
                     }
                 }
                 __syncwarp();
-                warp_bitonic(sm->key, sm->sid, P, lane);
+                warp_bitonic(sm->key(), sm->sid, P, lane);
             } else {
 #pragma unroll
                 for (int r = 0; r < E; ++r)
