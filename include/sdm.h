@@ -5,7 +5,7 @@
  * PAPER.md:<line>.  State of Fig. 2: per super-droplet a multiplicity xi
  * (int64), one extensive attribute, the volume v (fp64, m^3), and a cell id (int32).  Call order
  * and in/out intents follow Fig. 3.  Readings of the paper where it is silent
- * (RNG stream, tie rules, evaluation order, ...) are R1..R14 of DESIGN.md.
+ * (RNG stream, tie rules, evaluation order, ...) are R1..R17 of DESIGN.md.
  *
  * Conventions
  *  - Every entry point returns an int status: SDM_OK (0) or a negative SDM_E* code.  Nothing

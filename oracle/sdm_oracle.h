@@ -7,7 +7,7 @@
  * calls it.  Single-threaded, fp64, compiled with -O2 -ffp-contract=off (no FMA contraction).
  *
  * All pointers are HOST pointers.  Conventions where the paper is silent are the readings
- * R1..R14 of DESIGN.md ("Readings of the paper").
+ * R1..R17 of DESIGN.md ("Readings of the paper").
  *
  * Pins (tests/test_oracle_*.py): Philox known answers, the paper's worked example
  * (PAPER.md:106), the xi_k = 1 special case, hand-worked 4-droplet examples
