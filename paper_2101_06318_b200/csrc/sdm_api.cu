@@ -277,16 +277,17 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         // to cell_start2); when it did so last step, k_cell_start_sorted only rebuilds the table if a
         // compaction has moved droplets since (device flag), else it returns at once
         if (produced) std::swap(h->cell_start, h->cell_start2);
+        const int gb_count = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32,
+                                      h->ctas_per_sm > 0 ? h->ctas_per_sm : kCountBlocksPerSM);
         SDM_LAUNCH(h, k_cell_start_sorted, grid_for(h, (n_ub + 4 * kCellStartQuads - 1) / (4 * kCellStartQuads), 256, 8), 256, 0, h->cell, h->ctrl, h->n_cell,
-                   h->cell_start, produced ? 0 : 1);
+                   h->cell_start, produced ? 0 : 1, gb_count * kCountWarps);
         // shape of the per-cell kernel: E droplets per lane, L lanes per cell (capacity E*L).  Eight
         // droplets per lane keep the unrolled network inside the instruction cache; wider shapes lose
         // more to instruction fetch than they save in shuffles (measured).
         const bool bucket = h->max_count <= kCountCap &&
                             (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
         if (bucket) {
-            const int gb = grid_for(h, (int64_t)h->n_cell * 32, kCountWarps * 32,
-                                    h->ctas_per_sm > 0 ? h->ctas_per_sm : kCountBlocksPerSM);
+            const int gb = gb_count;
 #define SDM_COUNT(MM, TT)                                                                                      \
     SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<MM, TT>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,  \
                             h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm, h->part0,    \

@@ -302,9 +302,11 @@ __device__ __forceinline__ void cell_boundary(int prev, int c, int i, int *__res
 }
 
 __global__ void __launch_bounds__(256)
-k_cell_start_sorted(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell,
-                    int *__restrict__ cell_start, int force)
+k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell,
+                    int *__restrict__ cell_start, int force, int ticket0)
 {
+    // re-arm the chunk ticket of the step kernel that follows (its first gridDim*warps chunks are pre-assigned)
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->cell_ticket = ticket0;
     // the previous step's kernel may already have derived this table from cell_id (sdm_fused_count.cuh,
     // cell_table_from_staged_ids); it is stale only if a compaction has moved droplets since
     if (!force && ctrl->table_dirty == 0) return;
