@@ -55,7 +55,7 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.cell_bits = take(((size_t)n_cell + 1) * 4);
     L.bucket_base = take(((size_t)n_cell + 1) * 4);
     L.bucket_start = take(((size_t)L.nb_max + 1) * 4);
-    L.bucket_cnt = take(((size_t)L.nb_max + 1) * 4);
+    L.bucket_cnt = take(((size_t)L.nb_max + 1) * 4 * kRankStride);   // rank counters, one per 32-byte sector
     L.tile_status = take((size_t)L.n_tiles * 8);
     L.scan_status = take((size_t)(((int64_t)n_cell + L.nb_max) / 2048 + 4) * 8);
     L.part0 = take((size_t)kMomentBlocks * 8);
@@ -341,8 +341,9 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     SDM_LAUNCH(h, k_gen_count, (split && h->n_cell <= kCellCountBins) ? grid_for(h, n_ub, 256, 8) : g, 256, 0, h->cell,
                h->ctrl, h->n_cell, split, h->cell_bits, h->bucket_base, h->cell_cnt, h->bucket_cnt, h->idx, prm);
     const int scan_tiles = (h->n_cell + kScanTile - 1) / kScanTile + (split ? (n_seg + kScanTile - 1) / kScanTile : 0);
-    SDM_LAUNCH(h, k_gen_scan, scan_tiles < 4 * h->num_sms ? scan_tiles : 4 * h->num_sms, kScanTileThreads, 0, h->cell_cnt,
-               h->n_cell, h->cell_start, split, h->bucket_cnt, n_seg, h->bucket_start, h->ctrl, h->scan_status);
+    SDM_LAUNCH(h, k_gen_scan, scan_tiles < 4 * h->num_sms ? scan_tiles : 4 * h->num_sms, kScanTileThreads, 0, split ? h->cell_cnt : h->bucket_cnt,
+               split ? 1 : kRankStride, h->n_cell, h->cell_start, split, h->bucket_cnt, kRankStride, n_seg,
+               h->bucket_start, h->ctrl, h->scan_status);
     SDM_LAUNCH(h, k_gen_scatter, g, 256, 0, h->cell, h->ctrl, split, h->cell_bits, h->bucket_base, seg_start,
                h->idx, h->order, prm);
     // four droplets per lane when no segment can exceed 128 (half the Philox blocks per warp), else eight
@@ -522,7 +523,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(spec)");
     e = cudaMemsetAsync(h->cell_cnt, 0, ((size_t)n_cell + 1) * 4, h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(cell_cnt)");
-    e = cudaMemsetAsync(h->bucket_cnt, 0, ((size_t)h->L.nb_max + 1) * 4, h->stream);
+    e = cudaMemsetAsync(h->bucket_cnt, 0, ((size_t)h->L.nb_max + 1) * 4 * kRankStride, h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(bucket_cnt)");
     e = cudaMemsetAsync(h->cell_start, 0, ((size_t)n_cell + 1) * 4, h->stream);
     if (e != cudaSuccess) return bail(e, "cudaMemsetAsync(cell_start)");

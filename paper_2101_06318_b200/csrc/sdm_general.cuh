@@ -21,6 +21,8 @@
 namespace sdmk {
 
 constexpr int kGenWarps = 8;
+constexpr int kRankStride = 8;             // rank counters sit one per 32-byte sector: L2 serialises the returning
+                                          // atomics that hit one sector (measured: k_gen_count 23 -> 8 us at 2^20)
 constexpr int kGenCap = 256;              // segment capacity of the warp counting sort
 
 struct __align__(1024) GenSmem {
@@ -117,7 +119,7 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[E], int m, int la
 // The split of large cells (cell_bits[c] = B key bits, bucket_base[c] = first segment of cell c) is
 // decided ONCE per loaded state from the cell counts (k_cell_scan with split = 1): cells never grow
 // (PAPER.md:9, 77), so the segments only get smaller afterwards, and idx does not depend on B.
-// Invariant between steps: cell_cnt[] and seg_cnt[] are all zero (the scan clears what it read).
+// Invariant between steps: cell_cnt[] and the rank counters are all zero (the scan clears what it read).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int segment_of(int c, uint32_t key_hi, const int *__restrict__ cell_bits,
                                           const int *__restrict__ bucket_base)
@@ -134,7 +136,7 @@ __device__ __forceinline__ int segment_of(int c, uint32_t key_hi, const int *__r
 __global__ void __launch_bounds__(256)
 k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int n_cell, int split,
             const int *__restrict__ cell_bits, const int *__restrict__ bucket_base,
-            int *__restrict__ cell_cnt, int *__restrict__ seg_cnt, int *__restrict__ rank,
+            int *__restrict__ cell_cnt, int *__restrict__ rank_cnt, int *__restrict__ rank,
             const __grid_constant__ StepParams prm)
 {
     __shared__ int s_cnt[kCellCountBins];
@@ -152,7 +154,7 @@ k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int
         const bool leader = (int)(__ffs(peers) - 1) == lane;
         if (!split) {                                   // segment == cell: the cell counter gives the rank
             int base = 0;
-            if (c >= 0 && leader) base = atomicAdd(&cell_cnt[c], __popc(peers));
+            if (c >= 0 && leader) base = atomicAdd(&rank_cnt[(size_t)c * kRankStride], __popc(peers));
             base = __shfl_sync(0xffffffffu, base, __ffs(peers) - 1);
             if (c >= 0) rank[i] = base + __popc(peers & ((1u << lane) - 1u));
         } else {
@@ -164,7 +166,7 @@ k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int
             }
             const unsigned speers = __match_any_sync(0xffffffffu, seg);
             int base = 0;
-            if (seg >= 0 && (int)(__ffs(speers) - 1) == lane) base = atomicAdd(&seg_cnt[seg], __popc(speers));
+            if (seg >= 0 && (int)(__ffs(speers) - 1) == lane) base = atomicAdd(&rank_cnt[(size_t)seg * kRankStride], __popc(speers));
             base = __shfl_sync(0xffffffffu, base, __ffs(speers) - 1);
             if (seg >= 0) rank[i] = base + __popc(speers & ((1u << lane) - 1u));
         }
@@ -185,8 +187,8 @@ constexpr int kScanTile = 2048;
 constexpr int kScanTileThreads = 256;
 
 __global__ void __launch_bounds__(kScanTileThreads)
-k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start, int split,
-           int *__restrict__ seg_cnt, int n_seg, int *__restrict__ seg_start, Ctrl *ctrl,
+k_gen_scan(int *__restrict__ cell_cnt, int cell_stride, int n_cell, int *__restrict__ cell_start, int split,
+           int *__restrict__ seg_cnt, int seg_stride, int n_seg, int *__restrict__ seg_start, Ctrl *ctrl,
            unsigned long long *__restrict__ status)
 {
     constexpr int kItems = kScanTile / kScanTileThreads;          // 8
@@ -205,6 +207,7 @@ k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start,
         if (tile >= tiles_a + tiles_b) break;
         const bool second = tile >= tiles_a;
         int *cnt = second ? seg_cnt : cell_cnt;
+        const size_t stride = second ? seg_stride : cell_stride;
         int *start = second ? seg_start : cell_start;
         const int m = second ? n_seg : n_cell;
         const int chain0 = second ? tiles_a : 0;                  // first tile of this chain
@@ -212,7 +215,7 @@ k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start,
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             const int e = k * kScanTileThreads + tid;
-            s_val[e + (e >> 5)] = (base + e < m) ? cnt[base + e] : 0;
+            s_val[e + (e >> 5)] = (base + e < m) ? cnt[(size_t)(base + e) * stride] : 0;
         }
         __syncthreads();
         int loc[kItems], sum = 0;
@@ -270,7 +273,7 @@ k_gen_scan(int *__restrict__ cell_cnt, int n_cell, int *__restrict__ cell_start,
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             const int e = k * kScanTileThreads + tid;
-            if (base + e < m) { start[base + e] = s_val[e + (e >> 5)]; cnt[base + e] = 0; }
+            if (base + e < m) { start[base + e] = s_val[e + (e >> 5)]; cnt[(size_t)(base + e) * stride] = 0; }
         }
         if (tid == 0 && base + kScanTile >= m) start[m] = s_prefix + tile_total;      // the chain's last tile
     }
