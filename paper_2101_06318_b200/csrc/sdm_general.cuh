@@ -52,12 +52,17 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[E], int m, int la
     uint32_t old[E];
 #pragma unroll
     for (int k = 0; k < E; ++k) {
-        const bool valid = nrem > L * k;
-        const uint4 w = droplet_block((uint32_t)id[k], step, rk);
-        const uint32_t hi = __funnelshift_l(w.x, w.y, shift);          // top 32 bits of key64 << shift
-        x[k] = valid ? ((hi & ~(uint32_t)(N - 1)) | (uint32_t)(lane + L * k)) : 0xFFFFFFFFu;
+        x[k] = 0xFFFFFFFFu;
         old[k] = 0;
-        if (valid) old[k] = atoms_add(sm_base | ((hi >> 22) & 0x3FCu), 4u);
+        if (L * k < m) {                                               // warp-uniform: rows beyond the segment cost nothing
+            const bool valid = nrem > L * k;
+            const uint4 w = droplet_block((uint32_t)id[k], step, rk);
+            const uint32_t hi = __funnelshift_l(w.x, w.y, shift);      // top 32 bits of key64 << shift
+            if (valid) {
+                x[k] = (hi & ~(uint32_t)(N - 1)) | (uint32_t)(lane + L * k);
+                old[k] = atoms_add(sm_base | ((hi >> 22) & 0x3FCu), 4u);
+            }
+        }
     }
     __syncwarp();
     uint32_t rounds;
