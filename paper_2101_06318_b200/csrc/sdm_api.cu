@@ -288,15 +288,23 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                             (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
         if (bucket) {
             const int gb = gb_count;
-#define SDM_COUNT(MM, TT)                                                                                      \
-    SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<MM, TT>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,  \
-                            h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm, h->part0,    \
+#define SDM_COUNT_K(MM, TT, KK)                                                                                   \
+    SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<MM, TT, KK>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,   \
+                            h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm, h->part0,        \
                             h->part1, h->part2, m0, m1, m2))
+#define SDM_COUNT(MM, TT)                                                                                         \
+    do {                                                                                                          \
+        if (tickets) SDM_COUNT_K(MM, TT, true);                                                                   \
+        else SDM_COUNT_K(MM, TT, false);                                                                          \
+    } while (0)
             const bool tab = prm.kernel == SDM_KERNEL_GRAVITATIONAL_TABULATED;
+            // chunk tickets pay off when a warp gets many chunks; small tables keep the static stride
+            const bool tickets = (int64_t)h->n_cell >= (int64_t)32 * gb * kCountWarps;
             if (m0 && tab) SDM_COUNT(true, true);
             else if (m0) SDM_COUNT(true, false);
             else if (tab) SDM_COUNT(false, true);
             else SDM_COUNT(false, false);
+#undef SDM_COUNT_K
 #undef SDM_COUNT
             h->table_produced = true;
             return SDM_OK;
@@ -507,10 +515,16 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     e = cudaFuncSetAttribute(k_segment_sort_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_segment_sort_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGenSmemBytes);
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_segment_sort_pairs)");
-    e = cudaFuncSetAttribute(k_fused_cells_count<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_cells_count<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCountSmemBytes);
+    e = cudaSuccess;
+#define SDM_SMEM_ATTR(MM, TT, KK)                                                                              \
+    if (e == cudaSuccess)                                                                                      \
+        e = cudaFuncSetAttribute(k_fused_cells_count<MM, TT, KK>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                                 (int)kCountSmemBytes)
+    SDM_SMEM_ATTR(true, false, true); SDM_SMEM_ATTR(false, false, true);
+    SDM_SMEM_ATTR(true, true, true); SDM_SMEM_ATTR(false, true, true);
+    SDM_SMEM_ATTR(true, false, false); SDM_SMEM_ATTR(false, false, false);
+    SDM_SMEM_ATTR(true, true, false); SDM_SMEM_ATTR(false, true, false);
+#undef SDM_SMEM_ATTR
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count)");
     if (n_attr > 1) {
         e = cudaFuncSetAttribute(k_compact, cudaFuncAttributeMaxDynamicSharedMemorySize,

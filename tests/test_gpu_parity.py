@@ -163,13 +163,14 @@ def test_cell_table_from_the_step_kernel_survives_removals_and_empty_cells(sdm_m
     s.close()
 
 
-@pytest.mark.parametrize("ctas_per_sm", [1, 3])
-def test_cell_tickets_with_other_grid_sizes(sdm_mod, ctas_per_sm):
-    """The counting-sort kernel hands cells out by chunk tickets whose first chunks are pre-assigned per warp:
-    the result must not depend on the grid (fewer CTAs than SMs x 2, or more CTAs than can be resident)."""
-    w = workloads.grid_uniform(40, 40, 256, seed=9)
+@pytest.mark.parametrize("ctas_per_sm,edge,steps", [(1, 200, 2), (3, 40, 4)])
+def test_cell_scheduling_with_other_grid_sizes(sdm_mod, ctas_per_sm, edge, steps):
+    """The counting-sort kernel hands cells out by chunk tickets when the table is large (>= 32 cells per warp of
+    the grid: 200 x 200 cells on one CTA per SM) and by a static stride otherwise; the result must not depend on
+    the grid (fewer CTAs than SMs x 2, or more CTAs than can be resident)."""
+    w = workloads.grid_uniform(edge, edge, 256, seed=9)
     w.dV = 0.5
-    events, _ = _run_parity(sdm_mod, w, 4, options=[(sdm_mod.OPT_CTAS_PER_SM, ctas_per_sm)], expect_mode=1)
+    events, _ = _run_parity(sdm_mod, w, steps, options=[(sdm_mod.OPT_CTAS_PER_SM, ctas_per_sm)], expect_mode=1)
     assert events > 500
 
 
