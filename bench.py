@@ -91,7 +91,7 @@ class ClockSampler:
 
     def __init__(self, gpu_index: int):
         self.gpu = gpu_index
-        self.sm, self.bits, self.max_mhz = [], 0, None
+        self.sm, self.power, self.bits, self.max_mhz = [], [], 0, None
         self.stop_flag = threading.Event()
         self.thread = None
         self.error = None
@@ -122,6 +122,7 @@ class ClockSampler:
             try:
                 self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
                 self.bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception as e:                 # noqa: BLE001
                 self.error = str(e)
                 return
@@ -134,14 +135,34 @@ class ClockSampler:
         self.thread.join(timeout=5)
         reasons = [name for name, attr in self.REASONS if self.bits & int(getattr(self.nv, attr, 0))]
         return {"sm_mhz": statistics.median(self.sm) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "sm_mhz_min": min(self.sm) if self.sm else None,
+                "power_w": statistics.median(self.power) if self.power else None,
+                "power_w_max": max(self.power) if self.power else None,
                 "samples": len(self.sm), "reasons": reasons}
 
 
-def oracle_sample_rate(target_s: float = 12.0):
-    """The oracle as it stands, one thread, on a bounded C5-shaped sample (64x64 cells x 256)."""
+def cpu_info():
+    """CPU model string and core count of the box the oracle is timed on (SURVEY.md 8(d) "Oracle timing")."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return model, os.cpu_count()
+
+
+def oracle_sample_rate(target_s: float = 12.0, full: bool = False):
+    """The oracle as it stands, one thread, on a bounded C5-shaped sample (64x64 cells x 256), or -- with
+    --cpu-baseline-full -- three steps of the full-size C5 state (about a minute of CPU work)."""
     import oracle
     import workloads
-    w = workloads.grid_uniform(64, 64, 256, seed=0)
+    w = workloads.grid_uniform(512, 512, 256, seed=0) if full else workloads.grid_uniform(64, 64, 256, seed=0)
+    if full:
+        target_s = 1e9
     xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
     steps, t0 = 0, time.perf_counter()
     while True:
@@ -150,7 +171,7 @@ def oracle_sample_rate(target_s: float = 12.0):
         oracle.moments(xi, v)
         steps += 1
         el = time.perf_counter() - t0
-        if el >= target_s or steps >= 200:
+        if el >= target_s or steps >= (3 if full else 200):
             break
     return w.n_sd * steps / el, steps, w.n_sd, el
 
@@ -178,14 +199,16 @@ def run_reference(args):
         one(args.warmup + s)
     el = time.perf_counter() - t0
     value = w.n_sd * args.steps / el
-    sample = "C5-shaped sample: 64x64 cells x 256 droplets (2^20) per step, single thread"
+    model, nproc = cpu_info()
+    sample = f"C5-shaped sample: 64x64 cells x 256 droplets (2^20) per step, single thread on {model} ({nproc} cores)"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / max(args.steps, 1),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "C5: 512x512 cells x 256 droplets, gravitational kernel (reference arm runs a bounded sample)",
                    "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "cpu_model": model, "nproc": nproc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -202,6 +225,8 @@ def main():
     ap.add_argument("--cells", type=int, default=None, help="C5 only: grid edge (default 512)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-full", action="store_true",
+                    help="time the oracle on 3 steps of the full-size C5 state instead of the 2^20 sample (~1 min)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, help="tuning: lanes per cell of the fused kernel (0 = auto)")
     ap.add_argument("--ctas-per-sm", type=int, default=0, help="tuning: grid of the counting-sort kernel (0 = auto)")
@@ -343,9 +368,11 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        rate, osteps, on, oel = oracle_sample_rate()
-        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"C5-shaped sample: 64x64 cells x 256 droplets (n_sd={on}), {osteps} steps in {oel:.1f} s, single thread"}
+        rate, osteps, on, oel = oracle_sample_rate(full=args.cpu_baseline_full)
+        model, nproc = cpu_info()
+        shape = "full C5 state: 512x512" if args.cpu_baseline_full else "C5-shaped sample: 64x64"
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "cpu_model": model, "nproc": nproc,
+               "sample": f"{shape} cells x 256 droplets (n_sd={on}), {osteps} steps in {oel:.1f} s, single thread"}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

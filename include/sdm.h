@@ -57,8 +57,11 @@ enum {
     SDM_OPT_LANES_PER_CELL = 6, /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)         */
     SDM_OPT_SORT_ENGINE = 7,   /* [0] fused path, per-cell permutation: 0 automatic, 1 register sorting  */
                                /*     network, 2 bucket sort on the top key bits (cells <= 256 only)     */
-    SDM_OPT_SORT_FALLBACK = 8, /* [0] reserved (no effect)                                                */
-    SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count (scaling runs) */
+    SDM_OPT_DETERMINISTIC = 8, /* [0] 1: cells are mapped to warps by a fixed rule (no work tickets), so the  */
+                               /*     fp64 moment sums M1, M2 of sdm_coalescence_step_moments are reproducible */
+                               /*     bit for bit from run to run (xi, v, idx, M0 always are)                 */
+    SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count, at most 32      */
+                               /*     (scaling runs; SDM_EINVAL if the grid would exceed the moment partials)  */
 };
 
 /* Counter slots returned by sdm_get_counters. */
@@ -74,7 +77,9 @@ enum {
 };
 
 /* Bytes of device workspace needed for `capacity` super-droplets in `n_cell` cells; 0 if the
- * arguments are invalid (capacity < 1, capacity >= 2^31 - 1024, n_cell < 1). */
+ * arguments are invalid (capacity < 1, capacity > SDM_MAX_CAPACITY, n_cell < 1).  Storage indices are 32-bit
+ * inside the kernels; the bound leaves room for the grid-stride loops' last increment. */
+#define SDM_MAX_CAPACITY 2139095040 /* 2^31 - 2^23 */
 size_t sdm_workspace_bytes(int64_t capacity, int32_t n_cell);
 
 /* The same for a state with n_attr extensive attributes per super-droplet (1 <= n_attr <= SDM_MAX_ATTR):

@@ -18,7 +18,7 @@ from .binding import (  # noqa: F401
     OPT_TIMING,
     OPT_LANES_PER_CELL,
     OPT_SORT_ENGINE,
-    OPT_SORT_FALLBACK,
+    OPT_DETERMINISTIC,
     OPT_CTAS_PER_SM,
     load_library,
     library_path,

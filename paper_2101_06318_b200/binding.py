@@ -20,7 +20,7 @@ OPT_SCREENING = 4
 OPT_TIMING = 5
 OPT_LANES_PER_CELL = 6
 OPT_SORT_ENGINE = 7
-OPT_SORT_FALLBACK = 8
+OPT_DETERMINISTIC = 8
 OPT_CTAS_PER_SM = 9
 CNT_NAMES = ("n_sd", "events", "zeros", "launches", "mode", "max_cell", "exact_evals", "reserved")
 

@@ -3,6 +3,7 @@
 // workspace; the only host allocations are the handle and a small pinned read-back block.
 #include "../../include/sdm.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -58,9 +59,9 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.bucket_cnt = take(((size_t)L.nb_max + 1) * 4 * kRankStride);   // rank counters, one per 32-byte sector
     L.tile_status = take((size_t)L.n_tiles * 8);
     L.scan_status = take((size_t)(((int64_t)n_cell + L.nb_max) / 2048 + 4) * 8);
-    L.part0 = take((size_t)kMomentBlocks * 8);
-    L.part1 = take((size_t)kMomentBlocks * 8);
-    L.part2 = take((size_t)kMomentBlocks * 8);
+    L.part0 = take((size_t)kMomentPartials * 8);
+    L.part1 = take((size_t)kMomentPartials * 8);
+    L.part2 = take((size_t)kMomentPartials * 8);
     L.mom_out = take(3 * 8);
     L.ctrl = take(sizeof(Ctrl));
     L.spec = take((size_t)(4 * SDM_MAX_BINS + 1) * 8);          // spectrum: edges, widths, sums, result
@@ -105,6 +106,7 @@ struct sdm {
     int max_count = 0;           // largest cell at set_state (cells never grow afterwards)
     bool sorted = false;         // cell_id non-decreasing in storage (preserved by compaction)
     int num_sms = 148;
+    int device = 0;              // CUDA device of the workspace; every entry point runs with it current
     // options
     bool force_general = false;
     int seg_cap = kWarpCap;      // fused path: largest cell; general path: only when overridden (tests)
@@ -117,7 +119,7 @@ struct sdm {
     bool screening = true;
     int lanes_per_cell = 0;      // 0: automatic
     int sort_engine = 0;         // 0: automatic, 1: register sorting network, 2: bucket sort
-    bool sort_fallback = false;
+    bool deterministic = false;  // SDM_OPT_DETERMINISTIC: static cell -> warp mapping
     int ctas_per_sm = 0;         // 0: the kernel's own choice (tuning / scaling experiments)
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
@@ -138,6 +140,20 @@ int cuda_fail(sdm_t *h, cudaError_t e, const char *what)
 {
     return fail(h, SDM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
+
+// Entry points make the handle's device current for the duration of the call and restore the caller's.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; return; }
+        if (prev == dev) prev = -1; else cudaSetDevice(dev);
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define SDM_ENTER(h)                     \
+    if (!(h)) return SDM_EINVAL;         \
+    DeviceGuard device_guard_((h)->device)
 
 #define SDM_CUDA(h, call)                                         \
     do {                                                          \
@@ -238,7 +254,6 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.seed = seed;
     prm.step = step;
     prm.screening = h->screening ? 1 : 0;
-    prm.sort_fallback = h->sort_fallback ? 1 : 0;
     prm.attr = attr_view(h);
     philox_round_keys(seed, prm.rk);
     return SDM_OK;
@@ -288,6 +303,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
                             (h->sort_engine == 2 || (h->sort_engine == 0 && h->max_count > 128));
         if (bucket) {
             const int gb = gb_count;
+            if (m0 && gb > kMomentPartials) return fail(h, SDM_EINVAL, "grid exceeds the moment partials (lower SDM_OPT_CTAS_PER_SM)");
 #define SDM_COUNT_K(MM, TT, KK)                                                                                   \
     SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells_count<MM, TT, KK>), gb, kCountWarps * 32, kCountSmemBytes, h->xi, h->v,   \
                             h->cell, h->cell_start, h->cell_start2, h->n_cell, h->idx, h->ctrl, prm, h->part0,        \
@@ -299,7 +315,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     } while (0)
             const bool tab = prm.kernel == SDM_KERNEL_GRAVITATIONAL_TABULATED;
             // chunk tickets pay off when a warp gets many chunks; small tables keep the static stride
-            const bool tickets = (int64_t)h->n_cell >= (int64_t)32 * gb * kCountWarps;
+            const bool tickets = !h->deterministic && (int64_t)h->n_cell >= (int64_t)32 * gb * kCountWarps;
             if (m0 && tab) SDM_COUNT(true, true);
             else if (m0) SDM_COUNT(true, false);
             else if (tab) SDM_COUNT(false, true);
@@ -315,7 +331,7 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
         else if (h->max_count > 64) { E = 8; L = 16; }
         if (h->lanes_per_cell == 16 && h->max_count > 128 && h->max_count <= 256) { E = 16; L = 16; }
         const int64_t warps_needed = ((int64_t)h->n_cell * L + 31) / 32;
-        const int gf = grid_for(h, warps_needed * 32, kFusedWarps * 32, 8);
+        const int gf = std::min(grid_for(h, warps_needed * 32, kFusedWarps * 32, 8), kMomentPartials);
 #define SDM_FUSED_T(EE, LL, MM, TT)                                                                          \
     SDM_TIMED(h, SDM_LAUNCH(h, (k_fused_cells<EE, LL, MM, TT>), gf, kFusedWarps * 32, 0, h->xi, h->v,            \
                             h->cell_start, h->n_cell, h->idx, h->ctrl, prm, h->part0, h->part1, h->part2, m0,    \
@@ -438,7 +454,7 @@ int sdm_version(void) { return 1004; }
 
 size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
-    if (capacity < 1 || capacity >= (int64_t)0x7fffffff - 1024 || n_cell < 1 || n_attr < 1 || n_attr > SDM_MAX_ATTR)
+    if (capacity < 1 || capacity > (int64_t)SDM_MAX_CAPACITY || n_cell < 1 || n_attr < 1 || n_attr > SDM_MAX_ATTR)
         return 0;
     return make_layout(capacity, n_cell, n_attr).total;
 }
@@ -467,6 +483,10 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDevice (no CUDA device? there is no CPU fallback)");
+    cudaPointerAttributes pa{};                           // the handle lives on the device that owns the workspace
+    if (cudaPointerGetAttributes(&pa, workspace_dev) == cudaSuccess && pa.type == cudaMemoryTypeDevice) dev = pa.device;
+    else cudaGetLastError();
+    DeviceGuard device_guard_(dev);
     cudaDeviceProp prop{};
     e = cudaGetDeviceProperties(&prop, dev);
     if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceProperties");
@@ -479,6 +499,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->n_attr = n_attr;
     h->L = make_layout(capacity, n_cell, n_attr);
     h->num_sms = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
+    h->device = dev;
     const Layout &L = h->L;
     h->xi = reinterpret_cast<int64_t *>(h->ws + L.xi);
     h->v = reinterpret_cast<double *>(h->ws + L.v);
@@ -549,7 +570,7 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
 
 int sdm_destroy(sdm_t *h)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     cudaStreamSynchronize(h->stream);
     if (h->ctrl_host) cudaFreeHost(h->ctrl_host);
     for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
@@ -559,7 +580,7 @@ int sdm_destroy(sdm_t *h)
 
 int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     switch (option) {
     case SDM_OPT_FORCE_GENERAL: h->force_general = value != 0; h->tables_ready = false; return SDM_OK;
     case SDM_OPT_SEGMENT_CAP:
@@ -582,7 +603,7 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         if (value < 0 || value > 2) return fail(h, SDM_EINVAL, "sort engine: 0 (auto), 1 (network) or 2 (bucket)");
         h->sort_engine = (int)value;
         return SDM_OK;
-    case SDM_OPT_SORT_FALLBACK: h->sort_fallback = value != 0; return SDM_OK;
+    case SDM_OPT_DETERMINISTIC: h->deterministic = value != 0; return SDM_OK;
     case SDM_OPT_CTAS_PER_SM:
         if (value < 0 || value > 32) return fail(h, SDM_EINVAL, "CTAs per SM: 0 (automatic) .. 32");
         h->ctas_per_sm = (int)value;
@@ -593,7 +614,7 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
 
 int sdm_set_state(sdm_t *h, int64_t n_sd, const int64_t *xi_dev, const double *v_dev, const int32_t *cell_id_dev)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (n_sd < 0) return fail(h, SDM_EINVAL, "n_sd < 0");
     if (n_sd > h->capacity) return fail(h, SDM_ECAPACITY, "n_sd exceeds the capacity given to sdm_create");
     if (n_sd > 0 && (!xi_dev || !v_dev || !cell_id_dev)) return fail(h, SDM_EINVAL, "state pointer is NULL");
@@ -609,7 +630,7 @@ int sdm_set_state(sdm_t *h, int64_t n_sd, const int64_t *xi_dev, const double *v
 int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const double *v_host,
                        const int32_t *cell_id_host)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (n_sd < 0) return fail(h, SDM_EINVAL, "n_sd < 0");
     if (n_sd > h->capacity) return fail(h, SDM_ECAPACITY, "n_sd exceeds the capacity given to sdm_create");
     if (n_sd > 0 && (!xi_host || !v_host || !cell_id_host)) return fail(h, SDM_EINVAL, "state pointer is NULL");
@@ -624,7 +645,7 @@ int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const dou
 
 int sdm_set_cell_id(sdm_t *h, const int32_t *cell_id_dev)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     int rc = read_ctrl(h);
     if (rc != SDM_OK) return rc;
@@ -654,7 +675,7 @@ int sdm_set_cell_id(sdm_t *h, const int32_t *cell_id_dev)
 
 int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (n_r < 2 || n_r > SDM_MAX_EFF_GRID) return fail(h, SDM_EINVAL, "need 2 <= n_r <= SDM_MAX_EFF_GRID");
     if (!r_grid_host || !E_host) return fail(h, SDM_EINVAL, "table pointer is NULL");
     for (int i = 0; i < n_r; ++i) {
@@ -677,7 +698,7 @@ int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, c
 
 int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (h->n_attr < 2) return fail(h, SDM_EINVAL, "the handle was created with n_attr = 1");
     int rc = read_ctrl(h);
@@ -700,7 +721,7 @@ int sdm_set_attributes(sdm_t *h, const double *attr_dev, int64_t ld)
 
 int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (h->n_attr < 2) return fail(h, SDM_EINVAL, "the handle was created with n_attr = 1");
     int rc = read_ctrl(h);
@@ -717,7 +738,7 @@ int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld)
 
 static int get_state_impl(sdm_t *h, int64_t *n_sd, int64_t *xi, double *v, int32_t *cell, cudaMemcpyKind kind)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     int rc = read_ctrl(h);
     if (rc != SDM_OK) return rc;
@@ -745,7 +766,7 @@ int sdm_get_state_host(sdm_t *h, int64_t *n_sd, int64_t *xi_host, double *v_host
 
 int sdm_coalescence_step(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed, uint64_t step)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     StepParams prm;
     int rc = make_params(h, dt, dV, kernel, seed, step, prm);
@@ -758,7 +779,7 @@ int sdm_coalescence_step(sdm_t *h, double dt, double dV, const sdm_kernel_t *ker
 int sdm_coalescence_step_moments(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
                                  uint64_t step, int64_t *m0_dev, double *m1_dev, double *m2_dev)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (!m0_dev || !m1_dev || !m2_dev) return fail(h, SDM_EINVAL, "moment output pointer is NULL");
     StepParams prm;
@@ -771,7 +792,7 @@ int sdm_coalescence_step_moments(sdm_t *h, double dt, double dV, const sdm_kerne
 
 int sdm_remove_zero(sdm_t *h, int64_t *n_sd_out)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     int rc = enqueue_remove_zero(h);
     if (rc != SDM_OK) return rc;
@@ -786,7 +807,7 @@ int sdm_remove_zero(sdm_t *h, int64_t *n_sd_out)
 
 int sdm_moments(sdm_t *h, int per_cell, int64_t *m0_dev, double *m1_dev, double *m2_dev)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (!m0_dev || !m1_dev || !m2_dev) return fail(h, SDM_EINVAL, "moment output pointer is NULL");
     return enqueue_moments(h, per_cell, m0_dev, m1_dev, m2_dev);
@@ -794,7 +815,7 @@ int sdm_moments(sdm_t *h, int per_cell, int64_t *m0_dev, double *m1_dev, double 
 
 int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, double *m2_host)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (!m0_host || !m1_host || !m2_host) return fail(h, SDM_EINVAL, "moment output pointer is NULL");
     if (!per_cell) {
@@ -826,7 +847,7 @@ int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, 
 int sdm_spectrum(sdm_t *h, int32_t n_bins, const double *v_edges_host, const double *dlnr_host, double rho,
                  double V, int32_t n_smooth, double *out_host)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (n_bins < 1 || n_bins > SDM_MAX_BINS) return fail(h, SDM_EINVAL, "need 1 <= n_bins <= SDM_MAX_BINS");
     if (!v_edges_host || !dlnr_host || !out_host) return fail(h, SDM_EINVAL, "spectrum pointer is NULL");
@@ -850,7 +871,7 @@ int sdm_spectrum(sdm_t *h, int32_t n_bins, const double *v_edges_host, const dou
 
 int sdm_get_permutation(sdm_t *h, int32_t *idx_dev, int32_t *cell_start_dev)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (!h->stepped) return fail(h, SDM_ESTATE, "no permutation: call sdm_coalescence_step first");
     if (idx_dev) {
@@ -870,7 +891,7 @@ int sdm_get_permutation(sdm_t *h, int32_t *idx_dev, int32_t *cell_start_dev)
 int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed, uint64_t step0,
             int64_t n_steps, int remove_zero_each_step)
 {
-    if (!h) return SDM_EINVAL;
+    SDM_ENTER(h);
     if (!h->valid) return fail(h, SDM_ESTATE, "no valid state loaded");
     if (n_steps < 0) return fail(h, SDM_EINVAL, "n_steps < 0");
     StepParams prm;
@@ -891,7 +912,8 @@ int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t
 
 int sdm_get_timing(sdm_t *h, double *total_ms, int64_t *n_launches)
 {
-    if (!h || !total_ms || !n_launches) return SDM_EINVAL;
+    SDM_ENTER(h);
+    if (!total_ms || !n_launches) return SDM_EINVAL;
     SDM_CUDA(h, cudaStreamSynchronize(h->stream));
     double total = 0.0;
     int64_t count = 0;
@@ -909,7 +931,8 @@ int sdm_get_timing(sdm_t *h, double *total_ms, int64_t *n_launches)
 
 int sdm_get_counters(sdm_t *h, int64_t *counters_host)
 {
-    if (!h || !counters_host) return SDM_EINVAL;
+    SDM_ENTER(h);
+    if (!counters_host) return SDM_EINVAL;
     int rc = read_ctrl(h);
     if (rc != SDM_OK) return rc;
     for (int i = 0; i < SDM_CNT_COUNT; ++i) counters_host[i] = 0;

@@ -87,7 +87,7 @@ struct StepParams {
     int32_t write_idx;
     uint64_t seed, step;
     int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
-    int32_t sort_fallback;  // unused (kept for ABI stability of the option numbering)
+    int32_t pad_;
     AttrView attr;          // extra extensive attributes
     PhiloxKey rk;           // round keys of `seed`: kernels that take the parameters as __grid_constant__ read
                             // them straight from the constant bank instead of holding 20 registers

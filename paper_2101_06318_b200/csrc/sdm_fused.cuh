@@ -345,10 +345,13 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         {
             // words that share the truncated key differ by less than N (necessary, not sufficient:
             // the slow path re-checks); sorted ascending, so differences are non-negative
+            // (sentinel words behind the last droplet are all equal and excluded: position li*E + r exists iff r < l0)
             const uint32_t nx = __shfl_down_sync(0xffffffffu, x[0], 1);
-            uint32_t dmin = (li < L - 1) ? nx - x[E - 1] : 0xFFFFFFFFu;
+            const int l0 = n_s - E * li;
+            uint32_t dmin = (li < L - 1 && l0 > E) ? nx - x[E - 1] : 0xFFFFFFFFu;
 #pragma unroll
-            for (int r = 0; r + 1 < E; ++r) dmin = min(dmin, x[r + 1] - x[r]);
+            for (int r = 0; r + 1 < E; ++r)
+                if (l0 > r + 1) dmin = min(dmin, x[r + 1] - x[r]);
             if (__any_sync(0xffffffffu, dmin < (uint32_t)N)) {
                 uint32_t *sk = s_scratch[warp][g];
 #pragma unroll

@@ -10,7 +10,9 @@ constexpr int kWarpCap = 512;            // largest segment one warp sorts in sh
 constexpr int kSortWarps = 8;            // warps per CTA in the segment kernels
 constexpr int kCompactTile = 2048;       // elements per compaction tile
 constexpr int kCompactThreads = 256;
-constexpr int kMomentBlocks = 1184;      // 148 SMs x 8
+constexpr int kMomentBlocks = 1184;      // grid of k_moments_global: 148 SMs x 8
+constexpr int kMomentPartials = 8192;    // per-CTA moment partials (part0..2): the largest grid of ANY kernel that
+                                         // ends in moments_finish; every such launch is checked against it on the host
 constexpr int kMomentThreads = 256;
 constexpr int kCellStartQuads = 4;       // k_cell_start_sorted: 16-byte loads per thread and round
 

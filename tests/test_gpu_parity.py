@@ -419,16 +419,58 @@ def test_every_shape_of_the_fused_kernel(sdm_mod, max_count, lanes):
     assert events > 50
 
 
-@pytest.mark.parametrize("max_count,engine,fallback", [(256, 2, 0), (256, 1, 0), (200, 2, 0), (100, 2, 0),
-                                                       (31, 2, 0), (256, 2, 1), (77, 2, 1)])
-def test_sort_engines_of_the_fused_kernel(sdm_mod, max_count, engine, fallback):
+@pytest.mark.parametrize("max_count,engine", [(256, 2), (256, 1), (200, 2), (100, 2), (31, 2)])
+def test_sort_engines_of_the_fused_kernel(sdm_mod, max_count, engine):
     """Per-cell permutation by bucket sort on the top key bits (engine 2) or by the register sorting
-    network (engine 1): both must reproduce the oracle's argsort by (key64, storage index); the
-    bucket sort's histogram-overflow fallback is forced through SDM_OPT_SORT_FALLBACK."""
+    network (engine 1): both must reproduce the oracle's argsort by (key64, storage index)."""
     rng = np.random.default_rng(1000 + max_count + engine)
     counts = rng.integers(0, max_count + 1, 53)
     counts[3], counts[7], counts[19], counts[52] = max_count, 1, 0, max_count
     w = _ragged_workload(counts, seed=max_count + engine, shuffled=False, kparam=0.3 / max_count)
-    opts = [(sdm_mod.OPT_SORT_ENGINE, engine), (sdm_mod.OPT_SORT_FALLBACK, fallback)]
+    opts = [(sdm_mod.OPT_SORT_ENGINE, engine)]
     events, _ = _run_parity(sdm_mod, w, 5, options=opts, expect_mode=1)
     assert events > 50
+
+
+def test_many_ctas_per_sm_with_fused_moments(sdm_mod):
+    """SDM_OPT_CTAS_PER_SM up to 32 launches up to 148 x 32 CTAs, each writing one moment partial: the partial
+    buffers must hold the largest grid (round-1 advisor finding: 1184 entries overflowed above 8 CTAs per SM)."""
+    w = workloads.grid_uniform(96, 96, 256, seed=5)
+    w.dV = 0.5
+    s = _make(sdm_mod, w, options=[(sdm_mod.OPT_CTAS_PER_SM, 32)])
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    for step in range(3):
+        xi, v, cell, _ = _compare_step(s, xi, v, cell, w, step, fused_moments=True)
+    assert s.counters()["n_sd"] == len(xi)
+    with pytest.raises(sdm_mod.SdmError):
+        s.set_option(sdm_mod.OPT_CTAS_PER_SM, 33)
+    s.close()
+
+
+def test_deterministic_option_makes_fused_moments_bit_reproducible(sdm_mod):
+    """With SDM_OPT_DETERMINISTIC the cell -> warp mapping is fixed, so M1 and M2 of
+    sdm_coalescence_step_moments are identical bit for bit between two runs of the same steps (a table large
+    enough for the ticket scheduler otherwise: 200 x 200 cells on one CTA per SM)."""
+    w = workloads.grid_uniform(200, 200, 256, seed=3)
+    w.dV = 5.0
+    runs = []
+    for rep in range(2):
+        s = _make(sdm_mod, w, options=[(sdm_mod.OPT_CTAS_PER_SM, 1), (sdm_mod.OPT_DETERMINISTIC, 1)])
+        out = []
+        for step in range(4):
+            s.remove_zero(sync=False)
+            m = s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+            out.append(tuple(t.cpu().numpy().tobytes() for t in m))
+        runs.append((out, tuple(t.cpu() for t in s.get_state())))
+        s.close()
+    assert runs[0][0] == runs[1][0]
+    for a, b in zip(runs[0][1], runs[1][1]):
+        assert torch.equal(a, b)
+    # and the same state as the default (ticket) schedule
+    s = _make(sdm_mod, w, options=[(sdm_mod.OPT_CTAS_PER_SM, 1)])
+    for step in range(4):
+        s.remove_zero(sync=False)
+        s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    for a, b in zip(runs[0][1], s.get_state()):
+        assert torch.equal(a, b.cpu())
+    s.close()
