@@ -255,6 +255,13 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     prm.step = step;
     prm.screening = h->screening ? 1 : 0;
     prm.attr = attr_view(h);
+    auto float_ru = [](double x) {                      // smallest fp32 >= x (inf stays inf)
+        float f = (float)x;
+        if ((double)f < x) f = std::nextafterf(f, INFINITY);
+        return f;
+    };
+    prm.dtdv_ub_f = float_ru(prm.dtdv);
+    prm.kparam_ub_f = float_ru(prm.kparam_ub);
     philox_round_keys(seed, prm.rk);
     return SDM_OK;
 }

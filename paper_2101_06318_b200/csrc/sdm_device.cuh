@@ -87,6 +87,8 @@ struct StepParams {
     int32_t write_idx;
     uint64_t seed, step;
     int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
+    float dtdv_ub_f;        // dt/dV and kparam_ub rounded UP to fp32 on the host (screening bounds only)
+    float kparam_ub_f;
     int32_t pad_;
     AttrView attr;          // extra extensive attributes
     PhiloxKey rk;           // round keys of `seed`: kernels that take the parameters as __grid_constant__ read
