@@ -228,8 +228,11 @@ def main():
     ap.add_argument("--cpu-baseline-full", action="store_true",
                     help="time the oracle on 3 steps of the full-size C5 state instead of the 2^20 sample (~1 min)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--per-step-calls", action="store_true",
+                    help="box workloads: time sdm_remove_zero + sdm_coalescence_step_moments per step instead of one sdm_run")
     ap.add_argument("--lanes", type=int, default=0, help="tuning: lanes per cell of the fused kernel (0 = auto)")
     ap.add_argument("--ctas-per-sm", type=int, default=0, help="tuning: grid of the counting-sort kernel (0 = auto)")
+    ap.add_argument("--box-ctas", type=int, default=0, help="tuning: CTAs of the persistent box kernel (0 = auto)")
     ap.add_argument("--engine", type=int, default=0, help="tuning: per-cell sort engine (0 auto, 1 network, 2 bucket)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -265,6 +268,8 @@ def main():
         s.set_option(pkg.OPT_SORT_ENGINE, args.engine)
     if args.ctas_per_sm:
         s.set_option(pkg.OPT_CTAS_PER_SM, args.ctas_per_sm)
+    if args.box_ctas:
+        s.set_option(pkg.OPT_BOX_CTAS, args.box_ctas)
     mode = s.counters()["mode"]
     mom = s.moments()
 
@@ -280,8 +285,19 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for st in range(args.warmup):
-        one_step(st)
+    # single-cell boxes (C1-C3): the paper's own benchmark is the 3600-step loop, which the library
+    # runs as ONE sdm_run call -- [remove_zero; step] x K inside one persistent launch -- followed by the moments
+    box_run = mode == 2 and not args.per_step_calls
+
+    def timed_steps(first, count):
+        if box_run:
+            s.run(w.dt, w.dV, w.kernel, w.kparam, seed, first, count, True)
+            s.moments(out=mom)
+        else:
+            for st in range(count):
+                one_step(first + st)
+
+    timed_steps(0, args.warmup)
     barrier()
     s.timing()                                   # drop warm-up kernel timings
     launches0 = s.counters()["launches"]
@@ -291,8 +307,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    for st in range(args.steps):
-        one_step(args.warmup + st)
+    timed_steps(args.warmup, args.steps)
     ev1.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -359,7 +374,8 @@ def main():
                                        "achieved": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9,
                                        "frac": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9 / peak}}
         else:
-            roofline = {"bound": "hbm", "kernel": "k_segment_sort (general path; L2-resident workload)",
+            roofline = {"bound": "hbm", "kernel": ("k_box_steps (persistent box kernel; L2-resident workload)" if mode == 2
+                                                   else "k_segment_sort (general path; L2-resident workload)"),
                         "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
                         "ms_per_launch": per_launch_s * 1e3, "launches_timed": kernel_n}
     # traffic: DRAM bytes per launch of the dominant kernel from the committed ncu summary (C5 only)
@@ -379,8 +395,9 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": wname, "n_sd_per_gpu": w.n_sd, "n_cell_per_gpu": w.n_cell,
-                   "step": "sdm_remove_zero + sdm_coalescence_step_moments (step + global moments)",
-                   "path": "fused cell-contiguous" if mode == 1 else "general",
+                   "step": ("one sdm_run(K steps, remove_zero each step) + sdm_moments: all K steps in one persistent launch"
+                            if box_run else "sdm_remove_zero + sdm_coalescence_step_moments (step + global moments)"),
+                   "path": {0: "general", 1: "fused cell-contiguous", 2: "single-cell box (persistent cooperative kernel)"}[mode],
                    "l2": "inputs larger than L2 (no flush)" if 20 * w.n_sd > 2 * 126e6 else "L2-resident workload (no flush; latency/launch-bound)",
                    "parallelism": f"cells sharded over {world} GPU(s), no data-path collective"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,

@@ -60,6 +60,8 @@ enum {
     SDM_OPT_DETERMINISTIC = 8, /* [0] 1: cells are mapped to warps by a fixed rule (no work tickets), so the  */
                                /*     fp64 moment sums M1, M2 of sdm_coalescence_step_moments are reproducible */
                                /*     bit for bit from run to run (xi, v, idx, M0 always are)                 */
+    SDM_OPT_BOX_CTAS = 10,     /* [0] >0: number of CTAs of the persistent box kernel (n_cell == 1; tuning), at   */
+                               /*     most the SM count; 0: chosen from the droplet count                          */
     SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count, at most 32      */
                                /*     (scaling runs; SDM_EINVAL if the grid would exceed the moment partials)  */
 };
@@ -70,7 +72,8 @@ enum {
     SDM_CNT_EVENTS = 1,      /* pairs with gamma_tilde > 0 since sdm_set_state                      */
     SDM_CNT_ZEROS = 2,       /* droplets with xi == 0 currently in the state                        */
     SDM_CNT_LAUNCHES = 3,    /* kernels launched by this handle since sdm_create                    */
-    SDM_CNT_MODE = 4,        /* 0 = general path, 1 = fused cell-contiguous path                    */
+    SDM_CNT_MODE = 4,        /* 0 = general path, 1 = fused cell-contiguous path, 2 = single-cell box  */
+                             /* path (n_cell == 1: all steps of a call in one persistent launch)      */
     SDM_CNT_MAX_CELL = 5,    /* largest per-cell count seen at sdm_set_state                        */
     SDM_CNT_EXACT_EVALS = 6, /* pairs whose Eq. 3 was evaluated in fp64 since sdm_set_state         */
     SDM_CNT_COUNT = 8

@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     OPT_SORT_ENGINE,
     OPT_DETERMINISTIC,
     OPT_CTAS_PER_SM,
+    OPT_BOX_CTAS,
     load_library,
     library_path,
     workspace_bytes,

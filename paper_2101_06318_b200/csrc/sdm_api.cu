@@ -20,6 +20,7 @@
 #include "sdm_fused_count.cuh"
 #include "sdm_general.cuh"
 #include "sdm_spectrum.cuh"
+#include "sdm_box.cuh"
 
 using namespace sdmk;
 
@@ -32,8 +33,8 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
     size_t xi, v, attr, eff, spec, cell, idx, order, cell_start, cell_start2, cell_cnt, cell_bits, bucket_base, bucket_start,
-        bucket_cnt, tile_status, scan_status, part0, part1, part2, mom_out, ctrl, total;
-    int64_t nb_max, n_tiles, attr_stride;
+        bucket_cnt, tile_status, scan_status, part0, part1, part2, mom_out, ctrl, box_ctrl, box_queue, total;
+    int64_t nb_max, n_tiles, attr_stride, box_stride;
 };
 
 Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
@@ -66,6 +67,14 @@ Layout make_layout(int64_t cap, int32_t n_cell, int32_t n_attr)
     L.ctrl = take(sizeof(Ctrl));
     L.spec = take((size_t)(4 * SDM_MAX_BINS + 1) * 8);          // spectrum: edges, widths, sums, result
     L.eff = take((size_t)(SDM_MAX_EFF_GRID + SDM_MAX_EFF_GRID * SDM_MAX_EFF_GRID) * 8);   // efficiency grid + table
+    // single-cell box path (sdm_box.cuh): control block and the double-buffered record queue, 2 x 8 B per droplet
+    L.box_stride = 0;
+    if (n_cell == 1 && cap <= (int64_t)kBoxMaxCtas * kBoxMeanMax) {
+        // fixed-capacity regions: G * (mean + 12 sqrt(mean) + 32) <= cap + 12 sqrt(255 cap) + 32 * 255 records
+        L.box_stride = ((int64_t)((double)cap + 12.0 * std::sqrt(255.0 * (double)cap)) + 8192 + 64) / 32 * 32;
+        L.box_ctrl = take(sizeof(BoxCtrl));
+        L.box_queue = take((size_t)2 * (size_t)L.box_stride * 8);
+    }
     L.total = off;
     return L;
 }
@@ -98,6 +107,9 @@ struct sdm {
     int64_t *mom0 = nullptr;
     double *mom1 = nullptr, *mom2 = nullptr;
     Ctrl *ctrl = nullptr;
+    BoxCtrl *box_ctrl = nullptr;                 // single-cell box path (nullptr: not available for this handle)
+    unsigned long long *box_queue = nullptr;
+    int box_max_ctas = 0;        // co-resident CTAs of k_box_steps on this device
     Ctrl *ctrl_host = nullptr;   // pinned read-back block
     // host knowledge of the state
     bool valid = false;          // a validated state is loaded
@@ -121,6 +133,7 @@ struct sdm {
     int sort_engine = 0;         // 0: automatic, 1: register sorting network, 2: bucket sort
     bool deterministic = false;  // SDM_OPT_DETERMINISTIC: static cell -> warp mapping
     int ctas_per_sm = 0;         // 0: the kernel's own choice (tuning / scaling experiments)
+    int box_ctas_opt = 0;        // SDM_OPT_BOX_CTAS
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
     size_t ev_used = 0;
@@ -203,9 +216,51 @@ inline int grid_for(const sdm_t *h, int64_t work, int block, int per_sm)
     return (int)g;
 }
 
+// single-cell box: persistent cooperative kernel (sdm_box.cuh); number of CTAs for the current droplet count, 0 = not usable
+int box_ctas(const sdm_t *h)
+{
+    if (!h->box_ctrl || h->force_general || h->seg_cap_set || h->box_max_ctas < 1) return 0;
+    const int64_t n = h->n_ub > 0 ? h->n_ub : 1;
+    int64_t g = (n + 511) / 512;                                // ~512 droplets per CTA for small boxes (measured: C1 best at 16 CTAs)
+    if (h->box_ctas_opt > 0) g = h->box_ctas_opt;
+    const int64_t cap = std::min<int64_t>(h->box_max_ctas, kBoxMaxCtas);
+    if (g > cap) g = cap;
+    if (n > g * kBoxMeanMax) return 0;
+    return (int)g;
+}
+
 bool use_fused(const sdm_t *h)
 {
     return h->sorted && !h->force_general && h->max_count <= h->seg_cap && h->max_count <= 512;
+}
+
+// [optional remove_zero; step] x n_steps of a single-cell state in one cooperative launch
+int enqueue_box(sdm_t *h, const StepParams &prm, int64_t n_steps, int remove_zero)
+{
+    const int g = box_ctas(h);
+    SDM_CUDA(h, cudaMemsetAsync(h->box_ctrl, 0, sizeof(BoxCtrl), h->stream));
+    StepParams p = prm;
+    while (n_steps > 0) {
+        int chunk = (int)std::min<int64_t>(n_steps, 1 << 20);
+        long long stride = h->L.box_stride;
+        // capacity of a region of the record queue: mean + 12 sigma (+ 32) of a Binomial(n, 1/G) count
+        const int64_t mean = (h->n_ub + g - 1) / g;
+        int region_cap = (int)(mean + (int64_t)(12.0 * std::sqrt((double)mean)) + 32);
+        if ((int64_t)region_cap * g > stride || region_cap > kBoxRegionMax)
+            return fail(h, SDM_EINVAL, "internal: box region capacity exceeds the workspace");
+        void *args[] = {&h->xi, &h->v, &h->cell, &h->idx, &h->cell_start, &h->ctrl, &h->box_ctrl, &h->box_queue, &stride,
+                        &region_cap, &h->tile_status, &chunk, &remove_zero, &p};
+        cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_box_steps, dim3(g), dim3(kBoxThreads), args, kBoxSmemBytes,
+                                                    h->stream);
+        h->launches += 1;
+        if (e != cudaSuccess) return cuda_fail(h, e, "launch k_box_steps");
+        n_steps -= chunk;
+        if (n_steps > 0) {
+            SDM_CUDA(h, cudaMemsetAsync(h->box_ctrl, 0, sizeof(BoxCtrl), h->stream));
+            p.step += (uint64_t)chunk;
+        }
+    }
+    return SDM_OK;
 }
 
 // largest segment of the general path: the warp counting sort holds 256 droplets
@@ -294,6 +349,11 @@ int enqueue_step(sdm_t *h, const StepParams &prm, int64_t *m0 = nullptr, double 
     const int64_t n_ub = h->n_ub;
     const bool produced = h->table_produced;      // did the previous step's kernel leave the next cell table?
     h->table_produced = false;
+    if (box_ctas(h) > 0) {
+        SDM_TIMED(h, { int rc_box = enqueue_box(h, prm, 1, 0); if (rc_box != SDM_OK) return rc_box; });
+        if (m0) return enqueue_moments(h, 0, m0, m1, m2);
+        return SDM_OK;
+    }
     if (use_fused(h)) {
         // row a2: the counting-sort kernel derives the NEXT step's table from cell_id while it runs (written
         // to cell_start2); when it did so last step, k_cell_start_sorted only rebuilds the table if a
@@ -532,6 +592,10 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     h->mom1 = reinterpret_cast<double *>(h->ws + L.mom_out + 8);
     h->mom2 = reinterpret_cast<double *>(h->ws + L.mom_out + 16);
     h->ctrl = reinterpret_cast<Ctrl *>(h->ws + L.ctrl);
+    if (L.box_stride > 0) {
+        h->box_ctrl = reinterpret_cast<BoxCtrl *>(h->ws + L.box_ctrl);
+        h->box_queue = reinterpret_cast<unsigned long long *>(h->ws + L.box_queue);
+    }
     auto bail = [&](cudaError_t ce, const char *what) {
         int rc = cuda_fail(nullptr, ce, what);
         if (h->ctrl_host) cudaFreeHost(h->ctrl_host);
@@ -554,6 +618,15 @@ int sdm_create_attr(sdm_t **out, int64_t capacity, int32_t n_cell, int32_t n_att
     SDM_SMEM_ATTR(true, true, false); SDM_SMEM_ATTR(false, true, false);
 #undef SDM_SMEM_ATTR
     if (e != cudaSuccess) return bail(e, "cudaFuncSetAttribute(k_fused_cells_count)");
+    if (h->box_ctrl) {
+        int coop = 0, per_sm = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        e = cudaFuncSetAttribute(k_box_steps, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBoxSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_box_steps, kBoxThreads, kBoxSmemBytes);
+        if (e != cudaSuccess) return bail(e, "k_box_steps attributes");
+        h->box_max_ctas = coop ? per_sm * h->num_sms : 0;
+    }
     if (n_attr > 1) {
         e = cudaFuncSetAttribute(k_compact, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)((SDM_MAX_ATTR - 1) * kCompactTile * 8));
@@ -611,6 +684,10 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         h->sort_engine = (int)value;
         return SDM_OK;
     case SDM_OPT_DETERMINISTIC: h->deterministic = value != 0; return SDM_OK;
+    case SDM_OPT_BOX_CTAS:
+        if (value < 0 || value > kBoxMaxCtas) return fail(h, SDM_EINVAL, "box CTAs: 0 (automatic) .. 255");
+        h->box_ctas_opt = (int)value;
+        return SDM_OK;
     case SDM_OPT_CTAS_PER_SM:
         if (value < 0 || value > 32) return fail(h, SDM_EINVAL, "CTAs per SM: 0 (automatic) .. 32");
         h->ctas_per_sm = (int)value;
@@ -904,6 +981,11 @@ int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t
     StepParams prm;
     int rc = make_params(h, dt, dV, kernel, seed, step0, prm);
     if (rc != SDM_OK) return rc;
+    if (box_ctas(h) > 0 && n_steps > 0) {
+        SDM_TIMED(h, { rc = enqueue_box(h, prm, n_steps, remove_zero_each_step ? 1 : 0); if (rc != SDM_OK) return rc; });
+        h->stepped = true;
+        return SDM_OK;
+    }
     for (int64_t s = 0; s < n_steps; ++s) {
         if (remove_zero_each_step) {
             rc = enqueue_remove_zero(h);
@@ -947,7 +1029,7 @@ int sdm_get_counters(sdm_t *h, int64_t *counters_host)
     counters_host[SDM_CNT_EVENTS] = (int64_t)h->ctrl_host->n_events;
     counters_host[SDM_CNT_ZEROS] = h->ctrl_host->zero_count;
     counters_host[SDM_CNT_LAUNCHES] = h->launches;
-    counters_host[SDM_CNT_MODE] = (h->valid && use_fused(h)) ? 1 : 0;
+    counters_host[SDM_CNT_MODE] = !h->valid ? 0 : (box_ctas(h) > 0 ? 2 : (use_fused(h) ? 1 : 0));
     counters_host[SDM_CNT_MAX_CELL] = h->max_count;
     counters_host[SDM_CNT_EXACT_EVALS] = (int64_t)h->ctrl_host->n_exact;
     if (h->valid) h->n_ub = h->ctrl_host->n;

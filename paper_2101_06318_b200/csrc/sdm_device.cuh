@@ -193,13 +193,14 @@ __device__ __forceinline__ double pair_norm(int n_s, double dtdv)
 // it for the built-in kernels: it runs at its register limit, and the mere presence of the table code in its
 // call graph cost 10 % (measured: 0.383 -> 0.421 ms on C5).
 // ---------------------------------------------------------------------------------------------
+// collide_pair_loaded: the same with the four values of the pair already in registers (callers that overlap the
+// loads of their next pair with the arithmetic of this one).
 template <bool TAB>
-__device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, double *__restrict__ v,
-                                                  int a, int b, double u, double norm,
-                                                  int32_t ktype, double kparam, const AttrView &av)
+__device__ __forceinline__ int collide_pair_loaded(int64_t *__restrict__ xi, double *__restrict__ v,
+                                                   int a, int b, int64_t xa, int64_t xb, double vj, double vk,
+                                                   double u, double norm, int32_t ktype, double kparam,
+                                                   const AttrView &av)
 {
-    int64_t xa = xi[a], xb = xi[b];
-    double vj = v[a], vk = v[b];                         // four independent loads, one round trip
     int j = a, k = b;
     int64_t xj = xa, xk = xb;
     if (xa < xb) {                                       // PAPER.md:257-259 (strict <, R8)
@@ -247,6 +248,16 @@ __device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, doub
         A[k] = t;
     }
     return half == 0 ? 3 : 1;
+}
+
+template <bool TAB>
+__device__ __forceinline__ int collide_pair_exact(int64_t *__restrict__ xi, double *__restrict__ v,
+                                                  int a, int b, double u, double norm,
+                                                  int32_t ktype, double kparam, const AttrView &av)
+{
+    const int64_t xa = xi[a], xb = xi[b];
+    const double va = v[a], vb = v[b];                   // four independent loads, one round trip
+    return collide_pair_loaded<TAB>(xi, v, a, b, xa, xb, va, vb, u, norm, ktype, kparam, av);
 }
 
 }  // namespace sdmk

@@ -383,35 +383,40 @@ k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell,
 // an older epoch and read as "not published", so the array never has to be cleared.
 constexpr unsigned long long kFlagAggregate = 1ull << 32, kFlagInclusive = 2ull << 32;
 
-__global__ void __launch_bounds__(kCompactThreads)
-k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
-          unsigned long long *__restrict__ status, const AttrView av)
+// The pass itself, as a device function, so that the persistent box kernel (sdm_box.cuh) can run it between two steps
+// of one launch: called by kCompactThreads threads of every CTA of the grid (tid = their index, n_ctas = the grid size);
+// `sync` synchronises exactly those threads (__syncthreads() in k_compact, a named barrier in the box kernel).
+struct CompactSmem {
+    int64_t s_xi[kCompactTile];
+    double s_v[kCompactTile];
+    int32_t s_c[kCompactTile];
+    int s_warp_cnt[kCompactThreads / 32];
+    int s_tile, s_prefix;
+};
+
+template <class Sync>
+__device__ __forceinline__ void compact_tiles(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell,
+                                              Ctrl *ctrl, unsigned long long *__restrict__ status, const AttrView &av,
+                                              CompactSmem &sm, double *s_extra, int tid, unsigned int n_ctas, Sync sync)
 {
-    extern __shared__ double s_extra[];                // av.n rows of kCompactTile values (extra attributes)
-    __shared__ int64_t s_xi[kCompactTile];
-    __shared__ double s_v[kCompactTile];
-    __shared__ int32_t s_c[kCompactTile];
-    __shared__ int s_warp_cnt[kCompactThreads / 32];
-    __shared__ int s_tile, s_prefix;
-    if (ctrl->zero_count == 0) return;                 // nothing to remove: every CTA leaves
-    const int n = ctrl->n;
-    const unsigned long long tag = (unsigned long long)(ctrl->epoch & 0x3fffffffu) << 34;
+    const int n = ((volatile Ctrl *)ctrl)->n;
+    const unsigned long long tag = (unsigned long long)(((volatile Ctrl *)ctrl)->epoch & 0x3fffffffu) << 34;
     const int n_tiles = (n + kCompactTile - 1) / kCompactTile;
-    const int tid = threadIdx.x, lane = lane_id(), warp = tid >> 5;
+    const int lane = tid & 31, warp = tid >> 5;
     constexpr int kItems = kCompactTile / kCompactThreads;      // 8
     constexpr int kWarpSpan = 32 * kItems;                       // 256 consecutive elements per warp
     while (true) {
-        __syncthreads();
-        if (tid == 0) s_tile = atomicAdd(&ctrl->ticket, 1);
-        __syncthreads();
-        const int tile = s_tile;
+        sync();
+        if (tid == 0) sm.s_tile = atomicAdd(&ctrl->ticket, 1);
+        sync();
+        const int tile = sm.s_tile;
         if (tile >= n_tiles) break;
         const int base = tile * kCompactTile;
         const int cnt = min(kCompactTile, n - base);
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             int e = k * kCompactThreads + tid;
-            if (e < cnt) { s_xi[e] = xi[base + e]; s_v[e] = v[base + e]; s_c[e] = cell[base + e]; }
+            if (e < cnt) { sm.s_xi[e] = xi[base + e]; sm.s_v[e] = v[base + e]; sm.s_c[e] = cell[base + e]; }
         }
         for (int r = 0; r < av.n; ++r) {                // staged BEFORE the tile publishes its count, like xi and v
             const double *A = av.p + (long long)r * av.stride + base;
@@ -421,22 +426,22 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
                 if (e < cnt) s_extra[r * kCompactTile + e] = A[e];
             }
         }
-        __syncthreads();
+        sync();
         unsigned masks[kItems];
         int wtotal = 0;
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             int e = warp * kWarpSpan + k * 32 + lane;
-            bool keep = (e < cnt) && (s_xi[e] != 0);
+            bool keep = (e < cnt) && (sm.s_xi[e] != 0);
             masks[k] = __ballot_sync(0xffffffffu, keep);
             wtotal += __popc(masks[k]);
         }
-        if (lane == 0) s_warp_cnt[warp] = wtotal;
-        __syncthreads();
+        if (lane == 0) sm.s_warp_cnt[warp] = wtotal;
+        sync();
         int woff = 0, tile_total = 0;
 #pragma unroll
         for (int w = 0; w < kCompactThreads / 32; ++w) {
-            int cw = s_warp_cnt[w];
+            int cw = sm.s_warp_cnt[w];
             if (w < warp) woff += cw;
             tile_total += cw;
         }
@@ -459,20 +464,20 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
                 vs[tile] = tag | kFlagInclusive | (unsigned long long)(excl + tile_total);
             }
             __threadfence();
-            s_prefix = excl;
+            sm.s_prefix = excl;
             if (tile == n_tiles - 1) ctrl->n_new = excl + tile_total;
         }
-        __syncthreads();
-        const int prefix = s_prefix;
+        sync();
+        const int prefix = sm.s_prefix;
         int run = woff;
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             int e = warp * kWarpSpan + k * 32 + lane;
             if ((masks[k] >> lane) & 1u) {
                 int dst = prefix + run + __popc(masks[k] & ((1u << lane) - 1u));
-                xi[dst] = s_xi[e];
-                v[dst] = s_v[e];
-                cell[dst] = s_c[e];
+                xi[dst] = sm.s_xi[e];
+                v[dst] = sm.s_v[e];
+                cell[dst] = sm.s_c[e];
                 for (int r = 0; r < av.n; ++r) av.p[(long long)r * av.stride + dst] = s_extra[r * kCompactTile + e];
             }
             run += __popc(masks[k]);
@@ -480,12 +485,12 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
     }
     // the last CTA to leave publishes the new count and re-arms the control block; every CTA has read
     // zero_count and n before it counts itself out, so nobody sees the new values half-way
-    __syncthreads();
+    sync();
     if (tid == 0) {
         __threadfence();
-        if (atomicAdd(&ctrl->compact_done, 1u) == gridDim.x - 1) {
+        if (atomicAdd(&ctrl->compact_done, 1u) == n_ctas - 1) {
             __threadfence();
-            ctrl->n = ((volatile Ctrl *)ctrl)->n_new;
+            ctrl->n = (n_tiles > 0) ? ((volatile Ctrl *)ctrl)->n_new : 0;
             ctrl->table_dirty = 1;
             ctrl->zero_count = 0;
             ctrl->ticket = 0;
@@ -493,6 +498,16 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
             ctrl->epoch = ctrl->epoch + 1u;
         }
     }
+}
+
+__global__ void __launch_bounds__(kCompactThreads)
+k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
+          unsigned long long *__restrict__ status, const AttrView av)
+{
+    extern __shared__ double s_extra[];                // av.n rows of kCompactTile values (extra attributes)
+    __shared__ CompactSmem sm;
+    if (ctrl->zero_count == 0) return;                 // nothing to remove: every CTA leaves
+    compact_tiles(xi, v, cell, ctrl, status, av, sm, s_extra, (int)threadIdx.x, gridDim.x, [] { __syncthreads(); });
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -79,10 +79,12 @@ def test_attributes_general_path_with_removal(sdm_mod):
     assert events > 3000 and n_end < w.n_sd
 
 
-def test_attributes_split_cell_box_and_max_rows(sdm_mod):
+@pytest.mark.parametrize("path", ["box", "general"])
+def test_attributes_single_cell_box_and_max_rows(sdm_mod, path):
     w = workloads.golovin_box(2 ** 12)
     w.kparam = 1500.0 * 200                                   # events from the first step on
-    events, _ = _run(sdm_mod, w, sdm_mod.binding.MAX_ATTR, 12, expect_mode=0)
+    opts, mode = ([(sdm_mod.OPT_FORCE_GENERAL, 1)], 0) if path == "general" else ([], 2)
+    events, _ = _run(sdm_mod, w, sdm_mod.binding.MAX_ATTR, 12, options=opts, expect_mode=mode)
     assert events > 500
 
 

@@ -81,11 +81,13 @@ def test_tabulated_kernel_fused_bitonic_kernel_and_screening_off(sdm_mod):
     assert a == b > 50
 
 
-def test_tabulated_kernel_general_path_box(sdm_mod):
+@pytest.mark.parametrize("path", ["box", "general"])
+def test_tabulated_kernel_single_cell_box(sdm_mod, path):
     w = workloads.gravitational_box(2 ** 14)
     w.dV = 1e6 / 256
     grid, E = _table(n_r=64, seed=2)
-    assert _run(sdm_mod, w, 8, grid, E, expect_mode=0) > 50
+    opts, mode = ([(sdm_mod.OPT_FORCE_GENERAL, 1)], 0) if path == "general" else ([], 2)
+    assert _run(sdm_mod, w, 8, grid, E, options=opts, expect_mode=mode) > 50
 
 
 def test_unit_table_reproduces_the_plain_gravitational_kernel(sdm_mod):

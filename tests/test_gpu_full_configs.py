@@ -175,7 +175,7 @@ def test_c1_golovin_box_2e13_all_3600_steps_and_closed_forms(sdm_mod, trajectori
     traj = trajectories["C1"]
     w = traj.w
     s = _load(sdm_mod, w)
-    assert s.counters()["mode"] == 0
+    assert s.counters()["mode"] == 2                          # single-cell box: the persistent box path
     m_init = s.moments_host()
     assert m_init[0] == 2 ** 23 * 10 ** 6
     xi, v, cell, _, _, events = _follow(s, traj, "C1", per_step_calls_at=(300,))
@@ -240,7 +240,7 @@ def test_c3_gravitational_box_2e20_100_steps(sdm_mod, trajectories):
     """Config 3 at its full size with the paper's dV: 100 steps against the oracle, every 25."""
     traj = trajectories["C3b"]
     s = _load(sdm_mod, traj.w)
-    assert s.counters()["mode"] == 0
+    assert s.counters()["mode"] == 2
     m1_0 = s.moments_host()[1]
     xi, v, cell, _, _, events = _follow(s, traj, "C3 2^20", per_step_calls_at=(25,))
     m = _moments_match(s, xi, v)

@@ -106,22 +106,92 @@ def test_c4_poisson_grid_shuffled_and_contiguous(sdm_mod):
         assert events > 50
 
 
-def test_c1_golovin_box_split_cell(sdm_mod):
+# A single-cell box takes the persistent box path (mode 2); SDM_OPT_FORCE_GENERAL sends it through the general path,
+# where the one cell of 8192 > 256 droplets is split into key buckets.  Both must give the oracle's result.
+def _box_path(sdm_mod, path):
+    return ([(sdm_mod.OPT_FORCE_GENERAL, 1)], 0) if path == "general" else ([], 2)
+
+
+@pytest.mark.parametrize("path", ["box", "general"])
+def test_c1_golovin_box(sdm_mod, path):
+    opts, mode = _box_path(sdm_mod, path)
     w = workloads.golovin_box(2 ** 13)
-    events, _ = _run_parity(sdm_mod, w, 40, expect_mode=0)      # one cell of 8192 > 512: bucketed sort
+    events, _ = _run_parity(sdm_mod, w, 40, options=opts, expect_mode=mode)
     assert events > 100
 
 
-def test_c2_golovin_box_2e17_few_steps(sdm_mod):
+@pytest.mark.parametrize("path", ["box", "general"])
+def test_c2_golovin_box_2e17_few_steps(sdm_mod, path):
+    opts, mode = _box_path(sdm_mod, path)
     w = workloads.golovin_box(2 ** 17)
-    _run_parity(sdm_mod, w, 3, expect_mode=0)
+    _run_parity(sdm_mod, w, 3, options=opts, expect_mode=mode)
 
 
-def test_c3_gravitational_box(sdm_mod):
+@pytest.mark.parametrize("path", ["box", "general"])
+def test_c3_gravitational_box(sdm_mod, path):
+    opts, mode = _box_path(sdm_mod, path)
     w = workloads.gravitational_box(2 ** 14)
     w.dV = 1e6 / 64                                            # denser box so that events occur early
-    events, _ = _run_parity(sdm_mod, w, 25, expect_mode=0)
+    events, _ = _run_parity(sdm_mod, w, 25, options=opts, expect_mode=mode)
     assert events > 20
+
+
+def _small_xi_box(n, seed, kparam):
+    rng = np.random.default_rng(seed)
+    xi = rng.integers(1, 4, n).astype(np.int64)
+    return workloads.Workload("small_xi_box", xi, rng.uniform(0.5, 2.0, n), np.zeros(n, dtype=np.int32), 1, 1.0, 1.0,
+                              workloads.configs.KERNEL_GOLOVIN, kparam, 0, seed=seed)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 1000, 1025, 5000, 40001])
+def test_box_path_sizes_with_removals_per_step_calls(sdm_mod, n):
+    """The persistent box kernel on ragged sizes (one CTA, two, many; odd counts; the odd one out), multiplicities 1..3
+    so that droplets vanish and sdm_remove_zero really compacts between the steps."""
+    w = _small_xi_box(n, 100 + n, 0.3 / max(n, 2))
+    events, n_end = _run_parity(sdm_mod, w, 8, expect_mode=2)
+    if n >= 1000:
+        assert events > n // 8 and n_end < n
+
+
+@pytest.mark.parametrize("n", [2, 999, 2048, 30000])
+def test_box_run_removes_zeros_inside_the_launch(sdm_mod, n):
+    """sdm_run on a box: all steps in ONE cooperative launch, zero removal (the stable compaction pass) inside it whenever a
+    multiplicity reached zero; state, permutation, counters equal the oracle's [remove_zero; step] loop, and the
+    per-step calls on the general path."""
+    w = _small_xi_box(n, 7 + n, 0.4 / n)
+    steps = 12
+    s = _make(sdm_mod, w)
+    assert s.counters()["mode"] == 2
+    launches0 = s.counters()["launches"]
+    s.run(w.dt, w.dV, w.kernel, w.kparam, w.seed, 0, steps, True)
+    assert s.counters()["launches"] == launches0 + 1
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    events = 0
+    for step in range(steps):
+        xi, v, cell = oracle.remove_zero(xi, v, cell)
+        idx, cs, nev = oracle.step(xi, v, cell, 1, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+        events += nev
+    gxi, gv, gc = (t.cpu().numpy() for t in s.get_state())
+    assert np.array_equal(gxi, xi) and np.array_equal(gv, v) and np.array_equal(gc, cell)
+    gidx, gcs = (t.cpu().numpy() for t in s.get_permutation(len(xi)))
+    assert np.array_equal(gidx, idx) and np.array_equal(gcs, cs)
+    cnt = s.counters()
+    assert cnt["events"] == events and cnt["n_sd"] == len(xi) and cnt["zeros"] == int((xi == 0).sum())
+    if n >= 999:
+        assert len(xi) < n                                   # droplets were removed inside the launch
+    g = _make(sdm_mod, w, options=[(sdm_mod.OPT_FORCE_GENERAL, 1)])
+    g.run(w.dt, w.dV, w.kernel, w.kparam, w.seed, 0, steps, True)
+    for a, b in zip(s.get_state(), g.get_state()):
+        assert torch.equal(a, b)
+    # without removal inside the launch: zeros stay in storage and keep taking part in the permutation (R11)
+    s2 = _make(sdm_mod, w)
+    s2.run(w.dt, w.dV, w.kernel, w.kparam, w.seed, 0, steps, False)
+    xi, v = w.xi.copy(), w.v.copy()
+    for step in range(steps):
+        oracle.step(xi, v, w.cell_id, 1, w.dt, w.dV, w.kernel, w.kparam, w.seed, step, want_perm=False)
+    gxi, gv, _ = (t.cpu().numpy() for t in s2.get_state())
+    assert np.array_equal(gxi, xi) and np.array_equal(gv, v)
+    s.close(), g.close(), s2.close()
 
 
 def test_c5_shape_gravitational_grid_fused(sdm_mod):
