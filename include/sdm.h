@@ -62,6 +62,10 @@ enum {
                                /*     bit for bit from run to run (xi, v, idx, M0 always are)                 */
     SDM_OPT_BOX_CTAS = 10,     /* [0] >0: number of CTAs of the persistent box kernel (n_cell == 1; tuning), at   */
                                /*     most the SM count; 0: chosen from the droplet count                          */
+    SDM_OPT_BOX_REGION_CAP = 11, /* [0] >0: capacity of a region of the box kernel's record queue (tests: a small value   */
+                               /*     forces the overflow fallback to exact region offsets)                             */
+    SDM_OPT_BOX_SORT_CAP = 12, /* [0] >0: largest region the box kernel sorts in shared memory (tests: a small value    */
+                               /*     forces the ranking-by-counting fallback in global memory)                        */
     SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count, at most 32      */
                                /*     (scaling runs; SDM_EINVAL if the grid would exceed the moment partials)  */
 };

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     OPT_DETERMINISTIC,
     OPT_CTAS_PER_SM,
     OPT_BOX_CTAS,
+    OPT_BOX_REGION_CAP,
+    OPT_BOX_SORT_CAP,
     load_library,
     library_path,
     workspace_bytes,

@@ -134,6 +134,7 @@ struct sdm {
     bool deterministic = false;  // SDM_OPT_DETERMINISTIC: static cell -> warp mapping
     int ctas_per_sm = 0;         // 0: the kernel's own choice (tuning / scaling experiments)
     int box_ctas_opt = 0;        // SDM_OPT_BOX_CTAS
+    int box_region_cap_opt = 0, box_sort_cap_opt = 0;   // SDM_OPT_BOX_REGION_CAP, SDM_OPT_BOX_SORT_CAP (tests)
     bool timing = false;
     std::vector<cudaEvent_t> ev;   // start/stop pairs around the dominant kernel (SDM_OPT_TIMING)
     size_t ev_used = 0;
@@ -248,8 +249,10 @@ int enqueue_box(sdm_t *h, const StepParams &prm, int64_t n_steps, int remove_zer
         int region_cap = (int)(mean + (int64_t)(12.0 * std::sqrt((double)mean)) + 32);
         if ((int64_t)region_cap * g > stride || region_cap > kBoxRegionMax)
             return fail(h, SDM_EINVAL, "internal: box region capacity exceeds the workspace");
+        if (h->box_region_cap_opt > 0) region_cap = std::min(region_cap, h->box_region_cap_opt);
+        int sort_cap = h->box_sort_cap_opt > 0 ? std::min(h->box_sort_cap_opt, kBoxRegionMax) : kBoxRegionMax;
         void *args[] = {&h->xi, &h->v, &h->cell, &h->idx, &h->cell_start, &h->ctrl, &h->box_ctrl, &h->box_queue, &stride,
-                        &region_cap, &h->tile_status, &chunk, &remove_zero, &p};
+                        &region_cap, &sort_cap, &h->tile_status, &chunk, &remove_zero, &p};
         cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_box_steps, dim3(g), dim3(kBoxThreads), args, kBoxSmemBytes,
                                                     h->stream);
         h->launches += 1;
@@ -684,6 +687,14 @@ int sdm_set_option(sdm_t *h, int32_t option, int64_t value)
         h->sort_engine = (int)value;
         return SDM_OK;
     case SDM_OPT_DETERMINISTIC: h->deterministic = value != 0; return SDM_OK;
+    case SDM_OPT_BOX_REGION_CAP:
+        if (value < 0 || value > kBoxRegionMax) return fail(h, SDM_EINVAL, "box region capacity: 0 (automatic) .. 9216");
+        h->box_region_cap_opt = (int)value;
+        return SDM_OK;
+    case SDM_OPT_BOX_SORT_CAP:
+        if (value < 0 || value > kBoxRegionMax) return fail(h, SDM_EINVAL, "box sort capacity: 0 (automatic) .. 9216");
+        h->box_sort_cap_opt = (int)value;
+        return SDM_OK;
     case SDM_OPT_BOX_CTAS:
         if (value < 0 || value > kBoxMaxCtas) return fail(h, SDM_EINVAL, "box CTAs: 0 (automatic) .. 255");
         h->box_ctas_opt = (int)value;

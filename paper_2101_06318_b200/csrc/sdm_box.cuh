@@ -129,7 +129,7 @@ __device__ __forceinline__ bool box_less_exact(unsigned long long a, unsigned lo
 __global__ void __launch_bounds__(kBoxThreads, 1)
 k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, int *__restrict__ idx,
             int *__restrict__ cell_start, Ctrl *ctrl, BoxCtrl *box, unsigned long long *__restrict__ queue,
-            long long queue_stride, int region_cap, unsigned long long *__restrict__ tile_status, int n_steps,
+            long long queue_stride, int region_cap, int sort_cap, unsigned long long *__restrict__ tile_status, int n_steps,
             int remove_zero,
             const __grid_constant__ StepParams prm)
 {
@@ -249,7 +249,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
         // ---------------- B: sort region c, idx, pairs ----------------
         const unsigned long long *qr = exact_layout ? q + my_off : q + (long long)c * region_cap;
         const double norm = pair_norm(n, prm.dtdv);
-        if (m > kBoxRegionMax) {
+        if (m > sort_cap) {
             // never with Philox keys (> 20 sigma); defined anyway: rank by counting in global memory
             for (int e = tid; e < m; e += kBoxThreads) {
                 const unsigned long long me = __ldcg(qr + e);
@@ -330,7 +330,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
         // rows a4-a6: pairs (2k, 2k+1) of the global order whose first member lies in this region; the loads of a
         // thread's next pair are issued before the arithmetic of the current one (L2 gathers: one round trip in all)
         if (m > 0) {
-            const bool big = m > kBoxRegionMax;
+            const bool big = m > sort_cap;
             if (big) __threadfence();
             auto members = [&](int e, int &a, int &b) -> bool {
                 if (e >= m || my_off + e + 1 >= n) return false;          // past the region, or the odd one out

@@ -153,6 +153,17 @@ def test_box_path_sizes_with_removals_per_step_calls(sdm_mod, n):
         assert events > n // 8 and n_end < n
 
 
+@pytest.mark.parametrize("option,value,n", [("OPT_BOX_REGION_CAP", 8, 5000), ("OPT_BOX_SORT_CAP", 16, 700),
+                                            ("OPT_BOX_CTAS", 1, 3000), ("OPT_BOX_CTAS", 148, 3000)])
+def test_box_fallback_paths_and_grid_sizes(sdm_mod, option, value, n):
+    """Paths of the box kernel that Philox keys never reach on their own: a region of the record queue that overflows
+    its fixed capacity (-> exact region offsets, second barrier) and a region too large for shared memory (-> ranking
+    by counting in global memory); plus a one-CTA grid and a grid with more CTAs than some regions have records."""
+    w = _small_xi_box(n, 31 + n, 0.3 / n)
+    events, n_end = _run_parity(sdm_mod, w, 6, options=[(getattr(sdm_mod, option), value)], expect_mode=2)
+    assert events > n // 10 and n_end < n
+
+
 @pytest.mark.parametrize("n", [2, 999, 2048, 30000])
 def test_box_run_removes_zeros_inside_the_launch(sdm_mod, n):
     """sdm_run on a box: all steps in ONE cooperative launch, zero removal (the stable compaction pass) inside it whenever a
