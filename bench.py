@@ -271,14 +271,23 @@ def main():
     if args.box_ctas:
         s.set_option(pkg.OPT_BOX_CTAS, args.box_ctas)
     mode = s.counters()["mode"]
-    mom = s.moments()
 
     from paper_2101_06318_b200 import sharding
-    seed = sharding.shard_seed(w.seed, rank)     # every rank owns its cells and its own Philox key
+    # N > 1: rank r holds cells [r, r+1) / N of ONE global state (weak scaling: every rank the same number of cells):
+    # same Philox seed everywhere, global storage indices through the index base (sdm_set_index_base), and the three
+    # global moments all-gathered and summed on the device inside every timed step.  Boxes (one cell) do not shard:
+    # replicas with their own seeds.
+    seed = w.seed if mode != 2 else sharding.shard_seed(w.seed, rank)
+    if mode != 2 and world > 1:
+        s.set_index_base(rank * w.n_sd)          # no multiplicity can reach zero in this workload (checked after the run)
+    dmom = sharding.DeviceMoments(dev, world)
+    mom = dmom.out
 
     def one_step(step):
         s.remove_zero(sync=False)
         s.coalescence_step_moments(w.dt, w.dV, w.kernel, w.kparam, seed, step, out=mom)
+        if world > 1:
+            dmom.reduce()
 
     def barrier():
         if dist is not None:
@@ -314,6 +323,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     kernel_ms, kernel_n = s.timing()
     cnt = s.counters()
+    if world > 1 and mode != 2 and cnt["n_sd"] != w.n_sd:
+        raise SystemExit("a shard lost droplets: the index bases would have had to be re-derived (sharding.rebase)")
     launches = cnt["launches"] - launches0
     if dist is not None:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
@@ -399,7 +410,9 @@ def main():
                             if box_run else "sdm_remove_zero + sdm_coalescence_step_moments (step + global moments)"),
                    "path": {0: "general", 1: "fused cell-contiguous", 2: "single-cell box (persistent cooperative kernel)"}[mode],
                    "l2": "inputs larger than L2 (no flush)" if 20 * w.n_sd > 2 * 126e6 else "L2-resident workload (no flush; latency/launch-bound)",
-                   "parallelism": f"cells sharded over {world} GPU(s), no data-path collective"},
+                   "parallelism": (f"cells sharded over {world} GPU(s) (one global state, same seed, index bases); no data-path "
+                                   "collective; global moments all-gathered (24 B per rank) and summed on the device every step"
+                                   if mode != 2 else f"{world} independent replica(s) of the box (own seeds)")},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
         "events_in_run": cnt["events"],
     }

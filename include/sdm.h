@@ -144,6 +144,16 @@ int sdm_get_attributes(sdm_t *h, double *attr_dev, int64_t ld);
 #define SDM_MAX_EFF_GRID 64
 int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, const double *E_host);
 
+/* Sharding (cells are independent): this handle holds the slice [base, base + n_sd) of a
+ * larger, cell-contiguous GLOBAL state.  The Philox counter of a droplet is its global storage index base + i (i its
+ * index in this handle), so a shard loaded with the same seed reproduces the unsharded run exactly: same xi, v, and
+ * idx_global = base + idx.  The stable compaction shifts the droplets of later shards, so after every sdm_remove_zero
+ * that removed something the caller re-derives each shard's base as the exclusive scan of the shards' survivor counts
+ * (paper_2101_06318_b200/sharding.py: rebase).  Default 0.  Stays until changed (sdm_set_state does not reset it).
+ * Host-side only (no device work).  Errors: SDM_EINVAL unless 0 <= base and base + capacity <= 2^32 (the counter's
+ * index word is 32 bits wide in the kernels). */
+int sdm_set_index_base(sdm_t *h, int64_t base);
+
 /* Replaces the cell ids of the super-droplets currently in storage (cell_id_dev[n_sd], storage order) -- the
  * hook for particle displacement, which the paper performs between coalescence steps and outside this API
  * ("cell_id ... updated before this block"; "multi-dimensional" use).

@@ -37,7 +37,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
-    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id",
+    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base",
 )
 MAX_ATTR = 8
 
@@ -82,6 +82,7 @@ def load_library() -> C.CDLL:
     L.sdm_get_attributes.argtypes = [vp, vp, i64]
     L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
     L.sdm_set_cell_id.argtypes = [vp, vp]
+    L.sdm_set_index_base.argtypes = [vp, i64]
     L.sdm_spectrum.argtypes = [vp, i32, vp, vp, dbl, dbl, i32, vp]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
@@ -222,6 +223,10 @@ class SDM:
         """New cell ids (int32 device tensor, storage order, current n_sd entries) after displacement."""
         self._dev(cell_id, self.torch.int32)
         self._check(self._lib.sdm_set_cell_id(self._h, self._p(cell_id)))
+
+    def set_index_base(self, base: int):
+        """Global storage index of this handle's droplet 0 (sharded runs; see sdm_set_index_base)."""
+        self._check(self._lib.sdm_set_index_base(self._h, int(base)))
 
     def set_attributes(self, attr):
         """Rows 1..n_attr-1 of the attribute block: a contiguous float64 device tensor [n_attr-1, n_sd]."""

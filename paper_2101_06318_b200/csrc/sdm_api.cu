@@ -133,6 +133,7 @@ struct sdm {
     int sort_engine = 0;         // 0: automatic, 1: register sorting network, 2: bucket sort
     bool deterministic = false;  // SDM_OPT_DETERMINISTIC: static cell -> warp mapping
     int ctas_per_sm = 0;         // 0: the kernel's own choice (tuning / scaling experiments)
+    uint32_t index_base = 0;     // sdm_set_index_base: global storage index of this handle's droplet 0
     int box_ctas_opt = 0;        // SDM_OPT_BOX_CTAS
     int box_region_cap_opt = 0, box_sort_cap_opt = 0;   // SDM_OPT_BOX_REGION_CAP, SDM_OPT_BOX_SORT_CAP (tests)
     bool timing = false;
@@ -320,7 +321,7 @@ int make_params(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint
     };
     prm.dtdv_ub_f = float_ru(prm.dtdv);
     prm.kparam_ub_f = float_ru(prm.kparam_ub);
-    philox_round_keys(seed, prm.rk);
+    philox_round_keys(seed, h->index_base, prm.rk);
     return SDM_OK;
 }
 
@@ -520,7 +521,7 @@ int load_state_common(sdm_t *h, int64_t n_sd)
 
 extern "C" {
 
-int sdm_version(void) { return 1004; }
+int sdm_version(void) { return 2000; }
 
 size_t sdm_workspace_bytes_attr(int64_t capacity, int32_t n_cell, int32_t n_attr)
 {
@@ -736,6 +737,15 @@ int sdm_set_state_host(sdm_t *h, int64_t n_sd, const int64_t *xi_host, const dou
         SDM_CUDA(h, cudaMemcpyAsync(h->cell, cell_id_host, (size_t)n_sd * 4, cudaMemcpyHostToDevice, h->stream));
     }
     return load_state_common(h, n_sd);
+}
+
+int sdm_set_index_base(sdm_t *h, int64_t base)
+{
+    SDM_ENTER(h);
+    if (base < 0 || base + h->capacity > ((int64_t)1 << 32))
+        return fail(h, SDM_EINVAL, "index base: need 0 <= base and base + capacity <= 2^32");
+    h->index_base = (uint32_t)base;
+    return SDM_OK;
 }
 
 int sdm_set_cell_id(sdm_t *h, const int32_t *cell_id_dev)

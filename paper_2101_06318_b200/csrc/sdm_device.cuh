@@ -16,10 +16,13 @@ namespace sdmk {
 // ---------------------------------------------------------------------------------------------
 struct PhiloxKey {          // the ten round keys, precomputed once per thread (uniform values)
     uint32_t k0[10], k1[10];
+    uint32_t base;          // storage index of the handle's droplet 0 in the GLOBAL state (sdm_set_index_base): the
+                            // Philox counter is base + local index, so a shard reproduces the unsharded stream
 };
 
-__host__ __device__ __forceinline__ void philox_round_keys(uint64_t seed, PhiloxKey &rk)
+__host__ __device__ __forceinline__ void philox_round_keys(uint64_t seed, uint32_t base, PhiloxKey &rk)
 {
+    rk.base = base;
     uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -44,10 +47,11 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
-// counter = {storage index lo, hi, step lo, hi}; storage index < 2^31 so the hi word is 0
+// counter = {global storage index lo, hi, step lo, hi}; global index = base + local index < 2^32 (checked by
+// sdm_set_index_base), so the hi word is 0
 __device__ __forceinline__ uint4 droplet_block(uint32_t sid, uint64_t step, const PhiloxKey &rk)
 {
-    return philox4x32_10(sid, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
+    return philox4x32_10(sid + rk.base, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
 }
 
 __device__ __forceinline__ uint64_t block_key64(const uint4 &w)

@@ -116,10 +116,10 @@ __device__ __forceinline__ uint32_t flag_threshold(double P)
 // Works on shared memory only, so that the caller's register arrays never
 // get their address taken.  Called by the whole warp (every group with its own cell).
 __device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int N, int s, int n_s, int li, uint64_t seed,
-                                          uint64_t step)
+                                          uint32_t base, uint64_t step)
 {
     PhiloxKey rk;
-    philox_round_keys(seed, rk);
+    philox_round_keys(seed, base, rk);
     uint32_t mine[32], dst[32];
     for (int r = 0; r < E; ++r) {
         const int p = li * E + r;
@@ -166,14 +166,14 @@ __device__ __forceinline__ void pair_moments(const int64_t *xi, const double *v,
 template <bool TAB>
 __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *sflag, int E, int L, int lane0,
                                             int64_t *xi, double *v, int s, int n_s, int li, double dtdv,
-                                            int32_t ktype, double kparam, uint64_t seed, uint64_t step,
+                                            int32_t ktype, double kparam, uint64_t seed, uint32_t base, uint64_t step,
                                             double *delta, const AttrView &av)
 {
     const uint32_t N = (uint32_t)(E * L);
     int64_t d0 = 0;
     double d1 = 0.0, d2 = 0.0;
     PhiloxKey rk;
-    philox_round_keys(seed, rk);
+    philox_round_keys(seed, base, rk);
     const double norm = pair_norm(n_s, dtdv);
     int packed = 0;                                   // events | zeros << 10 | exact << 20
     for (int m = 0; m < E / 2; ++m) {
@@ -209,11 +209,11 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 // sdm_set_state and cells never grow); this keeps the result defined anyway.  Whole warp, one cell.
 template <bool TAB>
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
-                                          double dtdv, int32_t ktype, double kparam, uint64_t seed,
+                                          double dtdv, int32_t ktype, double kparam, uint64_t seed, uint32_t base,
                                           uint64_t step, double *delta, const AttrView &av)
 {
     PhiloxKey rk;
-    philox_round_keys(seed, rk);
+    philox_round_keys(seed, base, rk);
     warp_rank_by_counting(nullptr, s, n_s, s, idx, step, rk, lane);
     __syncwarp();
     const double norm = pair_norm(n_s, dtdv);
@@ -269,7 +269,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
     const int warp = threadIdx.x >> 5, lane = lane_id();
     const int g = lane / L, li = lane % L, lane0 = g * L;
     PhiloxKey rk;
-    philox_round_keys(prm.seed, rk);
+    philox_round_keys(prm.seed, prm.rk.base, rk);
     int events = 0, zeros = 0, exact = 0;
     const int cells_per_round = gridDim.x * kFusedWarps * G;
     for (int cbase = (blockIdx.x * kFusedWarps + warp) * G; cbase < n_cell; cbase += cells_per_round) {
@@ -284,7 +284,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
                 const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
                 if (n2 <= N) continue;
                 const int pk = oversize_cell<TAB>(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
-                                             prm.seed, prm.step, my_delta, prm.attr);
+                                             prm.seed, prm.rk.base, prm.step, my_delta, prm.attr);
                 events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
                 if (MOM) {
                     a0 += __double_as_longlong(my_delta[0]);
@@ -357,7 +357,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
 #pragma unroll
                 for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
                 __syncwarp();
-                fix_key_ties(sk, E, N, s, n_s, li, prm.seed, prm.step);
+                fix_key_ties(sk, E, N, s, n_s, li, prm.seed, prm.rk.base, prm.step);
 #pragma unroll
                 for (int r = 0; r < E; ++r) x[r] = sk[li * E + r];
                 __syncwarp();
@@ -401,7 +401,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
             __syncwarp();
             const int pk = collide_flagged<TAB>(sk, s_flags[warp], E, L, lane0, xi, v, s, n_s, li, prm.dtdv,
-                                           prm.kernel, prm.kparam, prm.seed, prm.step, my_delta, prm.attr);
+                                           prm.kernel, prm.kparam, prm.seed, prm.rk.base, prm.step, my_delta, prm.attr);
             events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
             if (MOM) {
                 a0 += __double_as_longlong(my_delta[0]);

@@ -37,7 +37,7 @@ def test_no_torch_types_and_extern_c_in_header():
 
 
 def test_version_and_workspace_sizing(lib):
-    assert lib.sdm_version() == 1004
+    assert lib.sdm_version() == 2000
     assert lib.sdm_workspace_bytes(0, 1) == 0
     assert lib.sdm_workspace_bytes(10, 0) == 0
     assert lib.sdm_workspace_bytes(2 ** 31, 1) == 0

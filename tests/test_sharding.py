@@ -32,6 +32,11 @@ def test_partition_covers_every_cell_once_and_balances_droplets():
     assert all(p.sd_hi == 0 for p in sharding.partition_cells([0, 0], 2))
 
 
+def test_index_bases_are_the_exclusive_scan_of_the_counts():
+    assert sharding.index_bases([5, 0, 7, 3]) == [0, 5, 5, 12]
+    assert sharding.index_bases([]) == [] and sharding.rebase(10, 0, 1) == 0
+
+
 def test_shard_seeds_are_distinct_and_rank0_keeps_the_seed():
     seeds = {sharding.shard_seed(7, r) for r in range(64)}
     assert len(seeds) == 64 and sharding.shard_seed(7, 0) == 7
@@ -65,14 +70,20 @@ def _rank_main(rank, world, port, ret):
     try:
         w = workloads.grid_small_multiplicity(12, 12, 24, seed=5)
         xi, v, cell, n_local, _ = sharding.shard_state(w.xi, w.v, w.cell_id, w.n_cell, rank, world)
-        seed = sharding.shard_seed(w.seed, rank)
-        for step in range(4):
+        for step in range(6):
             xi, v, cell = oracle.remove_zero(xi, v, cell)
-            oracle.step(xi, v, cell, n_local, w.dt, w.dV, w.kernel, w.kparam, seed, step)
+            base = sharding.rebase(len(xi), rank, world)          # all-gather of the survivor counts
+            sid = base + np.arange(len(xi), dtype=np.int64)       # what sdm_set_index_base tells the device
+            oracle.step(xi, v, cell, n_local, w.dt, w.dV, w.kernel, w.kparam, w.seed, step, sid=sid)
         m0, m1, m2 = oracle.moments(xi, v)
+        ret[("state", rank)] = (xi.copy(), v.copy())
         g = sharding.allreduce_moments(torch.tensor([m0]), torch.tensor([m1], dtype=torch.float64),
                                        torch.tensor([m2], dtype=torch.float64))
         t = sharding.max_over_ranks(1.0 + rank)
+        dm = sharding.DeviceMoments("cpu", world)                 # the device-side variant bench.py uses (here on gloo)
+        dm.out[0][0], dm.out[1][0], dm.out[2][0] = m0, m1, m2
+        dm.reduce()
+        assert dm.values() == g
         ret[rank] = (m0, m1, m2, g, t)
     finally:
         dist.destroy_process_group()
@@ -86,10 +97,20 @@ def test_two_gloo_ranks_step_their_shards_and_allreduce_moments():
         ret = mgr.dict()
         mp.spawn(_rank_main, args=(world, port, ret), nprocs=world, join=True)
         out = dict(ret)
+    states = {k[1]: out.pop(k) for k in list(out) if isinstance(k, tuple)}
     assert set(out) == {0, 1}
     m0 = sum(out[r][0] for r in out)
     m1 = sum(out[r][1] for r in out)
     m2 = sum(out[r][2] for r in out)
+    # the sharded run IS the unsharded one: same seed, global storage indices re-derived after every removal
+    w = workloads.grid_small_multiplicity(12, 12, 24, seed=5)
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    for step in range(6):
+        xi, v, cell = oracle.remove_zero(xi, v, cell)
+        oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    assert np.array_equal(np.concatenate([states[0][0], states[1][0]]), xi)
+    assert np.array_equal(np.concatenate([states[0][1], states[1][1]]), v)
+    assert len(xi) < w.n_sd                                       # removals shifted the second shard's base
     for r in out:
         g0, g1, g2 = out[r][3]
         assert g0 == m0 and abs(g1 - m1) <= 1e-12 * m1 and abs(g2 - m2) <= 1e-12 * m2
