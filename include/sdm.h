@@ -36,7 +36,8 @@ typedef struct sdm sdm_t; /* opaque handle, owned by the library (host memory on
 enum { SDM_OK = 0, SDM_EINVAL = -1, SDM_ECAPACITY = -2, SDM_ECUDA = -3, SDM_ESTATE = -4 };
 
 /* Coalescence kernel a(v1, v2) of Eq. 1 / Eq. 3. */
-enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GRAVITATIONAL = 1, SDM_KERNEL_GRAVITATIONAL_TABULATED = 2 };
+enum { SDM_KERNEL_GOLOVIN = 0, SDM_KERNEL_GRAVITATIONAL = 1, SDM_KERNEL_GRAVITATIONAL_TABULATED = 2,
+       SDM_KERNEL_USER = 3 /* a(v1, v2) from caller-supplied CUDA source, sdm_set_kernel_source; b and E are ignored */ };
 typedef struct {
     int32_t type;     /* SDM_KERNEL_*                                                              */
     int32_t reserved; /* must be 0                                                                 */
@@ -153,6 +154,22 @@ int sdm_set_efficiency_table(sdm_t *h, int32_t n_r, const double *r_grid_host, c
  * Host-side only (no device work).  Errors: SDM_EINVAL unless 0 <= base and base + capacity <= 2^32 (the counter's
  * index word is 32 bits wide in the kernels). */
 int sdm_set_index_base(sdm_t *h, int64_t base);
+
+/* User-supplied kernel code for SDM_KERNEL_USER (the paper keeps the pair logic apart from "potentially user-supplied
+ * kernel code"; Fig. 8 runs a second kernel family through the same interface).
+ * cuda_src is CUDA C++ source text (host pointer, NUL-terminated) that defines
+ *     __device__ double sdm_user_kernel(double vj, double vk, const double *params);
+ * returning a(v_j, v_k) [m^3/s] for the pair's volumes, vj being the member with the larger multiplicity (first-in-pair
+ * on a tie), exactly what the built-in kernels receive; params points to the n_params (0..SDM_MAX_USER_PARAMS) doubles
+ * of params_host, copied into the workspace.  The source is compiled at run time (NVRTC, sm_100a, no FMA contraction:
+ * every * and + of the user's code is rounded separately, like the library's own arithmetic) into one module with the
+ * library's pair code (Eq. 3-6, Fig. 5); steps with SDM_KERNEL_USER build the permutation with the library's kernels and
+ * evaluate every candidate pair through it (no probability screening: the library knows no bound of user code).
+ * A user kernel that re-expresses a built-in one reproduces it bit for bit.  SYNCHRONOUS.  Errors: SDM_EINVAL (NULL
+ * source, bad n_params, compilation failed: sdm_last_error holds the compiler log), SDM_ECUDA (NVRTC or the module loader
+ * unavailable).  The kernel stays until replaced. */
+#define SDM_MAX_USER_PARAMS 16
+int sdm_set_kernel_source(sdm_t *h, const char *cuda_src, int32_t n_params, const double *params_host);
 
 /* Replaces the cell ids of the super-droplets currently in storage (cell_id_dev[n_sd], storage order) -- the
  * hook for particle displacement, which the paper performs between coalescence steps and outside this API

@@ -16,6 +16,7 @@ from .build import build as _build
 KERNEL_GOLOVIN = 0
 KERNEL_GRAVITATIONAL = 1
 KERNEL_GRAVITATIONAL_TABULATED = 2
+KERNEL_USER = 3
 
 _lib = None
 
@@ -42,6 +43,8 @@ def lib() -> C.CDLL:
         L.orc_set_efficiency_table.restype = C.c_int
         L.orc_efficiency.argtypes = [C.c_double, C.c_double]
         L.orc_efficiency.restype = C.c_double
+        L.orc_set_user_kernel.argtypes = [p, p, C.c_int32]
+        L.orc_set_user_kernel.restype = None
         L.orc_pair_probability.argtypes = [C.c_double, C.c_int64, C.c_int64, C.c_double, C.c_double]
         L.orc_pair_probability.restype = C.c_double
         L.orc_gamma_tilde.argtypes = [C.c_double, C.c_double, C.c_int64, C.c_int64]
@@ -127,6 +130,30 @@ def set_efficiency_table(r_grid, E):
     assert E.shape == (r_grid.shape[0], r_grid.shape[0])
     if lib().orc_set_efficiency_table(r_grid.shape[0], _ptr(r_grid), _ptr(E)) != 0:
         raise ValueError("invalid efficiency table")
+
+
+_user_lib = None   # keeps the compiled user kernel alive
+
+
+def set_user_kernel(c_source: str, params=()):
+    """KERNEL_USER: compiles ``c_source`` -- plain C defining ``double sdm_user_kernel(double vj, double vk, const double
+    *params)`` -- with gcc (-O2 -ffp-contract=off, like the oracle itself) and hands the function to the oracle as a
+    callback.  Test infrastructure: the GPU library receives the same text as CUDA source (NVRTC, --fmad=false)."""
+    import os
+    import subprocess
+    import tempfile
+
+    global _user_lib
+    d = tempfile.mkdtemp(prefix="orc_user_")
+    src, so = os.path.join(d, "user_kernel.c"), os.path.join(d, "libuser_kernel.so")
+    with open(src, "w") as f:
+        f.write("#include <math.h>\n" + c_source + "\n")
+    subprocess.run(["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared", "-o", so, src,
+                    "-lm"], check=True)
+    _user_lib = C.CDLL(so)
+    fn = C.cast(_user_lib.sdm_user_kernel, C.c_void_p)
+    par = np.ascontiguousarray(np.asarray(params, dtype=np.float64))
+    lib().orc_set_user_kernel(fn, _ptr(par) if par.size else None, int(par.size))
 
 
 def efficiency(rj: float, rk: float) -> float:

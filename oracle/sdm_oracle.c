@@ -201,8 +201,18 @@ double orc_efficiency(double rj, double rk)
     return e0 + u * d;                                /* along r_k                       */
 }
 
+static orc_user_kernel_fn orc_user_fn = NULL;
+static double orc_user_params[16];
+
+void orc_set_user_kernel(orc_user_kernel_fn fn, const double *params, int32_t n_params)
+{
+    orc_user_fn = fn;
+    for (int32_t i = 0; i < 16; ++i) orc_user_params[i] = (params && i < n_params) ? params[i] : 0.0;
+}
+
 double orc_kernel(int32_t type, double kparam, double vj, double vk)
 {
+    if (type == ORC_KERNEL_USER) return orc_user_fn(vj, vk, orc_user_params);
     if (type == ORC_KERNEL_GOLOVIN) {
         /* a(v1, v2) = b (v1 + v2) */
         double s = vj + vk;

@@ -25,7 +25,7 @@
 extern "C" {
 #endif
 
-enum { ORC_KERNEL_GOLOVIN = 0, ORC_KERNEL_GRAVITATIONAL = 1, ORC_KERNEL_GRAVITATIONAL_TABULATED = 2 };
+enum { ORC_KERNEL_GOLOVIN = 0, ORC_KERNEL_GRAVITATIONAL = 1, ORC_KERNEL_GRAVITATIONAL_TABULATED = 2, ORC_KERNEL_USER = 3 };
 
 /* Philox4x32-10 (Salmon et al. 2011), one block.  DESIGN.md R6. */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
@@ -49,6 +49,13 @@ double orc_cbrt_spec(double x);
 /* Coalescence kernel a(v_j, v_k) [m^3/s]: Golovin b*(v_j+v_k) or the
  * gravitational kernel of BASELINE.json config 3 (PAPER.md:326 gives no formula). */
 double orc_kernel(int32_t type, double kparam, double vj, double vk);
+
+/* NEXT-2, "potentially user-supplied kernel code" (second kernel family of Fig. 8):
+ * ORC_KERNEL_USER evaluates a(v_j, v_k) = fn(v_j, v_k, params) with a caller-supplied C function (v_j: the volume of the
+ * pair member with the larger multiplicity, as for the built-in kernels); kparam is ignored.  The function must be
+ * compiled without FMA contraction if its result is to be compared bit for bit.  One function per process. */
+typedef double (*orc_user_kernel_fn)(double vj, double vk, const double *params);
+void orc_set_user_kernel(orc_user_kernel_fn fn, const double *params, int32_t n_params);
 
 /* NEXT-2: user-supplied collection efficiency E(r_1, r_2) for ORC_KERNEL_GRAVITATIONAL_TABULATED
  * (a = kparam * E(r_j, r_k) * pi * (r_j + r_k)^2 * |w_j - w_k|): n_r x n_r table,

@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     KERNEL_GOLOVIN,
     KERNEL_GRAVITATIONAL,
     KERNEL_GRAVITATIONAL_TABULATED,
+    KERNEL_USER,
     OPT_FORCE_GENERAL,
     OPT_SEGMENT_CAP,
     OPT_WRITE_IDX,

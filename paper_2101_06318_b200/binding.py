@@ -13,6 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 KERNEL_GOLOVIN = 0
 KERNEL_GRAVITATIONAL = 1
 KERNEL_GRAVITATIONAL_TABULATED = 2
+KERNEL_USER = 3
 OPT_FORCE_GENERAL = 1
 OPT_SEGMENT_CAP = 2
 OPT_WRITE_IDX = 3
@@ -37,7 +38,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
-    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base",
+    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base", "sdm_set_kernel_source",
 )
 MAX_ATTR = 8
 
@@ -83,6 +84,7 @@ def load_library() -> C.CDLL:
     L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
     L.sdm_set_cell_id.argtypes = [vp, vp]
     L.sdm_set_index_base.argtypes = [vp, i64]
+    L.sdm_set_kernel_source.argtypes = [vp, C.c_char_p, i32, vp]
     L.sdm_spectrum.argtypes = [vp, i32, vp, vp, dbl, dbl, i32, vp]
     L.sdm_destroy.argtypes = [vp]
     L.sdm_set_option.argtypes = [vp, i32, i64]
@@ -223,6 +225,15 @@ class SDM:
         """New cell ids (int32 device tensor, storage order, current n_sd entries) after displacement."""
         self._dev(cell_id, self.torch.int32)
         self._check(self._lib.sdm_set_cell_id(self._h, self._p(cell_id)))
+
+    def set_kernel_source(self, cuda_src: str, params=()):
+        """CUDA source defining ``__device__ double sdm_user_kernel(double vj, double vk, const double *params)`` for
+        KERNEL_USER, compiled at run time (NVRTC); params: up to 16 floats."""
+        import numpy as np
+
+        par = np.ascontiguousarray(np.asarray(params, dtype=np.float64))
+        self._check(self._lib.sdm_set_kernel_source(self._h, cuda_src.encode(), int(par.size),
+                                                    par.ctypes.data_as(C.c_void_p) if par.size else None))
 
     def set_index_base(self, base: int):
         """Global storage index of this handle's droplet 0 (sharded runs; see sdm_set_index_base)."""

@@ -329,7 +329,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
         }
         // rows a4-a6: pairs (2k, 2k+1) of the global order whose first member lies in this region; the loads of a
         // thread's next pair are issued before the arithmetic of the current one (L2 gathers: one round trip in all)
-        if (m > 0) {
+        if (m > 0 && !prm.no_pairs) {
             const bool big = m > sort_cap;
             if (big) __threadfence();
             auto members = [&](int e, int &a, int &b) -> bool {

@@ -6,8 +6,17 @@
 // is also compiled with -fmad=false).  Citations: PAPER.md = arXiv 2101.06318; R* = DESIGN.md.
 #pragma once
 
+// This header is also compiled at run time by NVRTC (sdm_set_kernel_source: the pair kernel around user-supplied kernel
+// code, sdm_user_pairs.cuh), where the toolkit headers are not available.
+#ifdef __CUDACC_RTC__
+typedef signed int int32_t;
+typedef unsigned int uint32_t;
+typedef long long int64_t;
+typedef unsigned long long uint64_t;
+#else
 #include <cstdint>
 #include <cuda_runtime.h>
+#endif
 
 namespace sdmk {
 
@@ -81,6 +90,7 @@ struct AttrView {
     int eff_n;
     const double *eff_grid;
     const double *eff_tab;
+    const double *user_params;   // SDM_KERNEL_USER: the caller's parameter array (device), sdm_set_kernel_source
 };
 
 struct StepParams {
@@ -93,7 +103,7 @@ struct StepParams {
     int32_t screening;      // 1: per-cell probability screening (sdm_fused.cuh); 0: every pair in fp64
     float dtdv_ub_f;        // dt/dV and kparam_ub rounded UP to fp32 on the host (screening bounds only)
     float kparam_ub_f;
-    int32_t pad_;
+    int32_t no_pairs;       // 1: rows a1-a3 only (the permutation); the caller evaluates the pairs (SDM_KERNEL_USER)
     AttrView attr;          // extra extensive attributes
     PhiloxKey rk;           // round keys of `seed`: kernels that take the parameters as __grid_constant__ read
                             // them straight from the constant bank instead of holding 20 registers
@@ -154,6 +164,13 @@ __device__ __forceinline__ double collection_efficiency(const AttrView &av, doub
     return __dadd_rn(e0, __dmul_rn(u, __dsub_rn(e1, e0)));
 }
 
+#ifdef SDM_USER_KERNEL
+}  // namespace sdmk
+// user-supplied kernel code, defined further down in the same run-time translation unit
+__device__ double sdm_user_kernel(double vj, double vk, const double *params);
+namespace sdmk {
+#endif
+
 __device__ __forceinline__ double coalescence_kernel(int32_t type, double kparam, double vj, double vk)
 {
     if (type == 0) return __dmul_rn(kparam, __dadd_rn(vj, vk));       // Golovin
@@ -212,8 +229,12 @@ __device__ __forceinline__ int collide_pair_loaded(int64_t *__restrict__ xi, dou
         const double t = vj; vj = vk; vk = t;
     }
     if (xk == 0) return 0;                               // R11
+#ifdef SDM_USER_KERNEL
+    double K = sdm_user_kernel(vj, vk, av.user_params);     // SDM_KERNEL_USER: the only kernel of this translation unit
+#else
     double K = (TAB && ktype == 2) ? coalescence_kernel_tabulated(kparam, vj, vk, av)
                                    : coalescence_kernel(ktype, kparam, vj, vk);
+#endif
     double p = __dmul_rn(__dmul_rn(K, __ll2double_rn(xj)), norm);      // Eq. 3 in routine order (R3)
     double fl = floor(p);
     double gamma = (u < __dsub_rn(p, fl)) ? __dadd_rn(fl, 1.0) : fl;       // PAPER.md:102, R4

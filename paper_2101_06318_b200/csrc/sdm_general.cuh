@@ -324,6 +324,7 @@ __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, in
 {
     const double norm = pair_norm(n_s, prm.dtdv);
     int packed = 0;
+    if (prm.no_pairs) return 0;
     for (int e = ((s - cs) & 1) + 2 * lane; e + 1 < m; e += 64) {
         const int a = sorted[e], b = sorted[e + 1];
         const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
@@ -439,6 +440,7 @@ k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__rest
 {
     const int n = ctrl->n;
     int events = 0, zeros = 0, exact = 0;
+    if (prm.no_pairs) return;
     for (int seg = blockIdx.x * blockDim.x + threadIdx.x + 1; seg < n_seg; seg += gridDim.x * blockDim.x) {
         const int p = seg_start[seg];
         if (p >= n || seg_start[seg - 1] == p) continue;   // an empty predecessor: boundary p belongs to an earlier seg
