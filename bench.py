@@ -65,6 +65,15 @@ def build_workload(name: str, rank: int = 0, scale_cells: int | None = None):
     if name == "C5":
         nx = ny = scale_cells or 512
         return workloads.grid_uniform(nx, ny, 256, seed=rank), f"C5: {nx}x{ny} cells x 256 droplets, gravitational kernel, cell-contiguous"
+    if name == "C5s":
+        nx = ny = scale_cells or 512
+        return (workloads.grid_uniform(nx, ny, 256, seed=rank, shuffled=True),
+                f"C5s: {nx}x{ny} cells x 256 droplets, gravitational kernel, SHUFFLED storage (as after displacement)")
+    if name == "C5d":
+        nx = ny = scale_cells or 512
+        w = workloads.grid_uniform(nx, ny, 256, seed=rank)
+        w.dV = 1.0                                 # collision-dense: p ~ 2.6e-2 per pair, the screening flags most cells
+        return w, f"C5d: {nx}x{ny} cells x 256 droplets, gravitational kernel, dV = 1 (collision-dense), cell-contiguous"
     if name == "C4":
         return workloads.grid_poisson(shuffled=False, seed=rank), "C4: 128x128 cells, Poisson(64)/cell, Golovin, cell-contiguous"
     if name == "C4s":

@@ -332,35 +332,45 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
         if (m > 0 && !prm.no_pairs) {
             const bool big = m > sort_cap;
             if (big) __threadfence();
-            auto members = [&](int e, int &a, int &b) -> bool {
-                if (e >= m || my_off + e + 1 >= n) return false;          // past the region, or the odd one out
-                a = big ? ((volatile int *)idx)[my_off + e] : (int)(uint32_t)sm.rec0[e];
-                if (e + 1 < m) {
-                    b = big ? ((volatile int *)idx)[my_off + e + 1] : (int)(uint32_t)sm.rec0[e + 1];
-                } else {
-                    while (((volatile unsigned int *)box->first_tag[p])[next_nonempty] != (unsigned int)t + 1u) { }
-                    __threadfence();
-                    b = (int)(uint32_t)((volatile unsigned long long *)box->first_rec[p])[next_nonempty];
+            // state-wide probability screening (sdm_general.cuh): a first-in-pair droplet whose top uniform word exceeds
+            // the threshold leads a pair with gamma = 0 -- nothing of it is read
+            const uint32_t thr = screen_threshold(prm, screen_bound(ctrl), n);
+            // the next pair at or after position e (stride 2 * kBoxThreads) that passes the screening
+            auto next_pair = [&](int &e, int &a, int &b, uint4 &w) -> bool {
+                for (; e < m && my_off + e + 1 < n; e += 2 * kBoxThreads) {
+                    a = big ? ((volatile int *)idx)[my_off + e] : (int)(uint32_t)sm.rec0[e];
+                    w = droplet_block((uint32_t)a, step, rk);
+                    if (w.w > thr) continue;
+                    if (e + 1 < m) {
+                        b = big ? ((volatile int *)idx)[my_off + e + 1] : (int)(uint32_t)sm.rec0[e + 1];
+                    } else {
+                        while (((volatile unsigned int *)box->first_tag[p])[next_nonempty] != (unsigned int)t + 1u) { }
+                        __threadfence();
+                        b = (int)(uint32_t)((volatile unsigned long long *)box->first_rec[p])[next_nonempty];
+                    }
+                    return true;
                 }
-                return true;
+                return false;
             };
             int e = tid * 2 + (my_off & 1), a = 0, b = 0;
-            bool have = members(e, a, b);
+            uint4 w = make_uint4(0u, 0u, 0u, 0u);
+            bool have = next_pair(e, a, b, w);
             int64_t xa = 0, xb = 0;
             double va = 0.0, vb = 0.0;
             if (have) { xa = xi[a]; xb = xi[b]; va = v[a]; vb = v[b]; }
             while (have) {
                 e += 2 * kBoxThreads;
                 int a2 = 0, b2 = 0;
-                const bool have2 = members(e, a2, b2);
+                uint4 w2 = make_uint4(0u, 0u, 0u, 0u);
+                const bool have2 = next_pair(e, a2, b2, w2);
                 int64_t xa2 = 0, xb2 = 0;
                 double va2 = 0.0, vb2 = 0.0;
                 if (have2) { xa2 = xi[a2]; xb2 = xi[b2]; va2 = v[a2]; vb2 = v[b2]; }
-                const double u = block_uniform(droplet_block((uint32_t)a, step, rk));
-                const int r = collide_pair_loaded<true>(xi, v, a, b, xa, xb, va, vb, u, norm, prm.kernel, prm.kparam, prm.attr);
+                const int r = collide_pair_loaded<true>(xi, v, a, b, xa, xb, va, vb, block_uniform(w), norm, prm.kernel,
+                                                        prm.kparam, prm.attr);
                 events += r & 1; exact += 1;
                 if (r & 2) atomicAdd(&ctrl->zero_count, 1);   // rare; seen by the barrier of the next step
-                have = have2; a = a2; b = b2; xa = xa2; xb = xb2; va = va2; vb = vb2;
+                have = have2; a = a2; b = b2; w = w2; xa = xa2; xb = xb2; va = va2; vb = vb2;
             }
         }
         if (c == 0 && tid == 0) { cell_start[0] = 0; cell_start[1] = n; }

@@ -91,6 +91,8 @@ struct AttrView {
     const double *eff_grid;
     const double *eff_tab;
     const double *user_params;   // SDM_KERNEL_USER: the caller's parameter array (device), sdm_set_kernel_source
+    unsigned long long *v_max;   // Ctrl::v_max_bits: bit pattern of the largest volume in the state (screening bound of the
+                                 // general and box paths); raised by every event that produces a larger volume
 };
 
 struct StepParams {
@@ -252,6 +254,10 @@ __device__ __forceinline__ int collide_pair_loaded(int64_t *__restrict__ xi, dou
     const double gd = __ll2double_rn(g);
     double gv = __dmul_rn(gd, vj);
     double vnew = __dadd_rn(vk, gv);                     // both branches produce v_k + g v_j
+    {                                                    // keep the state-wide volume bound valid (rarely a new maximum)
+        const unsigned long long nb = (unsigned long long)__double_as_longlong(vnew);
+        if (nb > *(volatile unsigned long long *)av.v_max) atomicMax(av.v_max, nb);
+    }
     if (new_n > 0) {                                     // Eq. 5
         xi[j] = new_n;
         v[k] = vnew;

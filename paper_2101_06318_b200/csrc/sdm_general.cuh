@@ -314,20 +314,47 @@ k_gen_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, i
     }
 }
 
+// Probability screening without reading the pair (same argument as sdm_fused.cuh, with bounds over the WHOLE state instead
+// of the cell): gamma = 0 whenever the pair's uniform u >= P >= p, where P bounds Eq. 3 through the largest multiplicity
+// and the largest volume anywhere in the state (Ctrl::xi_max, Ctrl::v_max_bits) and the cell's own n_s.  A first-in-pair
+// droplet whose top uniform word exceeds the threshold leads a pair that provably does nothing: its xi and v -- a 32-byte
+// sector each for an 8-byte value in shuffled storage -- are never gathered.  Results are identical (tested with
+// SDM_OPT_SCREENING = 0).
+struct ScreenBound {
+    float v_ub, xi_ub;
+};
+__device__ __forceinline__ ScreenBound screen_bound(const Ctrl *ctrl)
+{
+    ScreenBound b;
+    b.v_ub = __double2float_ru(__longlong_as_double((long long)((volatile Ctrl *)ctrl)->v_max_bits));
+    b.xi_ub = __ll2float_ru(((volatile Ctrl *)ctrl)->xi_max);
+    return b;
+}
+__device__ __forceinline__ uint32_t screen_threshold(const StepParams &prm, const ScreenBound &b, int n_s)
+{
+    if (!prm.screening) return 0xFFFFFFFFu;
+    const int ratio = (n_s & 1) ? n_s : n_s - 1;
+    const float norm_ub = __fmul_ru(prm.dtdv_ub_f, (float)max(ratio, 0));
+    return flag_threshold_f(cell_probability_bound_f(prm.kernel, prm.kparam_ub_f, b.v_ub, b.xi_ub, norm_ub));
+}
+
 // Rows a4-a6 for the candidate pairs that lie inside one sorted segment [s, s+m) of the cell that
 // starts at cs and holds n_s droplets (Fig. 4: positions cs+2k, cs+2k+1 pair up).
 // sorted[e] = storage index at position s+e.  A pair whose second member is the first droplet of the
 // next segment is left to k_pairs_straddle.  Returns events | zeros << 10 | exact << 20 of this lane.
 __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, int cs, int n_s, int lane,
                                              int64_t *__restrict__ xi, double *__restrict__ v,
-                                             const StepParams &prm)
+                                             const StepParams &prm, const ScreenBound &sb)
 {
     const double norm = pair_norm(n_s, prm.dtdv);
     int packed = 0;
     if (prm.no_pairs) return 0;
+    const uint32_t thr = screen_threshold(prm, sb, n_s);
     for (int e = ((s - cs) & 1) + 2 * lane; e + 1 < m; e += 64) {
         const int a = sorted[e], b = sorted[e + 1];
-        const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
+        const uint4 w = droplet_block((uint32_t)a, prm.step, prm.rk);
+        if (w.w > thr) continue;                          // u >= P >= p: gamma = 0, nothing to read
+        const double u = block_uniform(w);
         const int r = collide_pair_exact<true>(xi, v, a, b, u, norm, prm.kernel, prm.kparam, prm.attr);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
@@ -356,6 +383,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
     __syncwarp();
     seg_cap = min(seg_cap, N);
     int packed_sum_ev = 0, packed_sum_z = 0, packed_sum_ex = 0;
+    const ScreenBound sb = screen_bound(ctrl);
     const int warps_total = gridDim.x * kGenWarps;
     for (int seg = blockIdx.x * kGenWarps + (threadIdx.x >> 5); seg < n_seg; seg += warps_total) {
         const int s = seg_start[seg];
@@ -369,7 +397,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
             warp_rank_by_counting(order + s, 0, m, s, idx, prm.step, rk, lane);
             __threadfence_block();
             __syncwarp();
-            pk = segment_pairs(idx + s, s, m, cs, n_s, lane, xi, v, prm);
+            pk = segment_pairs(idx + s, s, m, cs, n_s, lane, xi, v, prm, sb);
         } else if (m == 1) {
             if (lane == 0) idx[s] = id0;
             pk = 0;
@@ -415,7 +443,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
                 __syncwarp();
             }
             for (int e = lane; e < m; e += 32) idx[s + e] = sm->sid[e];
-            pk = segment_pairs(sm->sid, s, m, cs, n_s, lane, xi, v, prm);
+            pk = segment_pairs(sm->sid, s, m, cs, n_s, lane, xi, v, prm, sb);
             __syncwarp();                                 // ids[], sid[] and slot[] are rewritten by the next segment
         }
         packed_sum_ev += pk & 1023; packed_sum_z += (pk >> 10) & 1023; packed_sum_ex += pk >> 20;
@@ -441,6 +469,7 @@ k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__rest
     const int n = ctrl->n;
     int events = 0, zeros = 0, exact = 0;
     if (prm.no_pairs) return;
+    const ScreenBound sb = screen_bound(ctrl);
     for (int seg = blockIdx.x * blockDim.x + threadIdx.x + 1; seg < n_seg; seg += gridDim.x * blockDim.x) {
         const int p = seg_start[seg];
         if (p >= n || seg_start[seg - 1] == p) continue;   // an empty predecessor: boundary p belongs to an earlier seg
@@ -449,7 +478,9 @@ k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__rest
         if (cell[b] != c) continue;
         const int cs = cell_start[c];
         if ((p - 1 - cs) & 1) continue;                    // a is a second-in-pair
-        const double u = block_uniform(droplet_block((uint32_t)a, prm.step, prm.rk));
+        const uint4 w = droplet_block((uint32_t)a, prm.step, prm.rk);
+        if (w.w > screen_threshold(prm, sb, cell_start[c + 1] - cs)) continue;
+        const double u = block_uniform(w);
         const int r = collide_pair_exact<true>(xi, v, a, b, u, pair_norm(cell_start[c + 1] - cs, prm.dtdv), prm.kernel,
                                          prm.kparam, prm.attr);
         events += r & 1;

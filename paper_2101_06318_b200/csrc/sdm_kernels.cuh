@@ -34,6 +34,11 @@ struct Ctrl {
     int pad0[1];
     unsigned long long n_events;   // pairs with gamma_tilde > 0
     unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
+    // upper bounds over the WHOLE state for the probability screening of the general and box paths (sdm_general.cuh):
+    // xi never grows (Eq. 5-6), so the largest multiplicity at sdm_set_state stays a bound; volumes grow only in
+    // coalescence events, which raise v_max_bits (bit pattern of a positive double: ordered like the value)
+    long long xi_max;
+    unsigned long long v_max_bits;
     int scan_ticket;               // general path scan: tile ticket
     unsigned int scan_done;        // general path scan: CTAs that have left the kernel
     unsigned int scan_epoch;       // general path scan: tag of valid status words
@@ -50,6 +55,8 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
                           int *__restrict__ cell_cnt, Ctrl *ctrl)
 {
     int zeros = 0, bad = 0, unsorted = 0;
+    long long xmax = 0;
+    unsigned long long vmax = 0ull;
     for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n; i0 += gridDim.x * blockDim.x) {
         const int i = i0 + lane_id();
         int c = -1;
@@ -60,6 +67,8 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
             const bool ok = (c >= 0) && (c < n_cell) && (x >= 0) && (vol > 0.0) && (vol < CUDART_INF);
             if (!ok) { bad = 1; c = -1; }
             else {
+                xmax = max(xmax, (long long)x);
+                vmax = max(vmax, (unsigned long long)__double_as_longlong(vol));
                 zeros += (x == 0);
                 if (i > 0 && cell[i - 1] > c) unsorted = 1;
             }
@@ -70,10 +79,17 @@ __global__ void k_analyze(const int64_t *__restrict__ xi, const double *__restri
     zeros = __reduce_add_sync(0xffffffffu, zeros);
     bad = __any_sync(0xffffffffu, bad);
     unsorted = __any_sync(0xffffffffu, unsorted);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        xmax = max(xmax, __shfl_xor_sync(0xffffffffu, xmax, d));
+        vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, d));
+    }
     if (lane_id() == 0) {
         if (zeros) atomicAdd(&ctrl->zero_count, zeros);
         if (bad) atomicOr(&ctrl->invalid, 1);
         if (unsorted) atomicOr(&ctrl->unsorted, 1);
+        atomicMax(&ctrl->xi_max, xmax);
+        atomicMax(&ctrl->v_max_bits, vmax);
     }
 }
 

@@ -92,7 +92,7 @@ def grid_poisson(nx: int = 128, ny: int = 128, mean_per_cell: float = 64.0, shuf
 
 
 def grid_uniform(nx: int = 512, ny: int = 512, per_cell: int = 256, steps: int = 100, seed: int = 0,
-                 kernel: int = KERNEL_GRAVITATIONAL) -> Workload:
+                 kernel: int = KERNEL_GRAVITATIONAL, shuffled: bool = False) -> Workload:
     """C5: nx*ny cells x per_cell droplets, cell-contiguous storage, exponential volumes with mean
     radius 15 um, xi = 1e6 for every droplet, gravitational kernel E=1, dV=1e3, dt=1."""
     rng = np.random.default_rng(seed)
@@ -104,7 +104,11 @@ def grid_uniform(nx: int = 512, ny: int = 512, per_cell: int = 256, steps: int =
     xi = np.full(n, 10 ** 6, dtype=np.int64)
     cell = np.repeat(np.arange(n_cell, dtype=np.int32), per_cell)
     kparam = 1.0 if kernel == KERNEL_GRAVITATIONAL else 1500.0
-    return Workload(f"grid{nx}x{ny}x{per_cell}", xi, v, cell, n_cell, 1.0, 1e3, kernel, kparam, steps)
+    if shuffled:                      # storage order after displacement: droplets of a cell scattered
+        perm = rng.permutation(n)
+        cell, v, xi = np.ascontiguousarray(cell[perm]), np.ascontiguousarray(v[perm]), np.ascontiguousarray(xi[perm])
+    return Workload(f"grid{nx}x{ny}x{per_cell}{'_shuffled' if shuffled else ''}", xi, v, cell, n_cell, 1.0, 1e3, kernel,
+                    kparam, steps)
 
 
 def grid_small_multiplicity(nx: int = 64, ny: int = 64, per_cell: int = 32, steps: int = 50,
