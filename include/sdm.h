@@ -240,6 +240,13 @@ int sdm_get_permutation(sdm_t *h, int32_t *idx_dev, int32_t *cell_start_dev);
 int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
             uint64_t step0, int64_t n_steps, int remove_zero_each_step);
 
+/* Testing hook for row a3 (the tie rule R7 cannot be reached with Philox output): runs rows a2-a3 of one step on the
+ * current state with the CALLER'S 64-bit sort keys, keys_dev[n_sd] by storage index, in place of Philox words 0-1,
+ * through the very kernels a real step of this state would use (fused, general or box path, their truncated-key and
+ * equal-key branches included); no pair is evaluated and the state does not change.  The result is read with
+ * sdm_get_permutation: idx = argsort by (cell_id, key, storage index).  ASYNCHRONOUS. */
+int sdm_debug_permutation(sdm_t *h, const uint64_t *keys_dev);
+
 /* Reads SDM_CNT_COUNT counters into counters_host.  SYNCHRONOUS. */
 int sdm_get_counters(sdm_t *h, int64_t *counters_host);
 

@@ -38,7 +38,7 @@ SYMBOLS = (
     "sdm_coalescence_step", "sdm_coalescence_step_moments", "sdm_remove_zero", "sdm_moments", "sdm_moments_host",
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
-    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base", "sdm_set_kernel_source",
+    "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base", "sdm_set_kernel_source", "sdm_debug_permutation",
 )
 MAX_ATTR = 8
 
@@ -84,6 +84,7 @@ def load_library() -> C.CDLL:
     L.sdm_set_efficiency_table.argtypes = [vp, i32, vp, vp]
     L.sdm_set_cell_id.argtypes = [vp, vp]
     L.sdm_set_index_base.argtypes = [vp, i64]
+    L.sdm_debug_permutation.argtypes = [vp, vp]
     L.sdm_set_kernel_source.argtypes = [vp, C.c_char_p, i32, vp]
     L.sdm_spectrum.argtypes = [vp, i32, vp, vp, dbl, dbl, i32, vp]
     L.sdm_destroy.argtypes = [vp]
@@ -234,6 +235,11 @@ class SDM:
         par = np.ascontiguousarray(np.asarray(params, dtype=np.float64))
         self._check(self._lib.sdm_set_kernel_source(self._h, cuda_src.encode(), int(par.size),
                                                     par.ctypes.data_as(C.c_void_p) if par.size else None))
+
+    def debug_permutation(self, keys):
+        """Rows a2-a3 with caller-supplied sort keys (uint64 as an int64 device tensor, by storage index): the tie rule."""
+        self._dev(keys, self.torch.int64)
+        self._check(self._lib.sdm_debug_permutation(self._h, self._p(keys)))
 
     def set_index_base(self, base: int):
         """Global storage index of this handle's droplet 0 (sharded runs; see sdm_set_index_base)."""

@@ -122,7 +122,7 @@ __device__ __forceinline__ bool box_less_exact(unsigned long long a, unsigned lo
     const uint32_t ha = (uint32_t)(a >> 32), hb = (uint32_t)(b >> 32);
     if (ha != hb) return ha < hb;
     const uint32_t ia = (uint32_t)a, ib = (uint32_t)b;
-    const uint32_t la = droplet_block(ia, step, rk).x, lb = droplet_block(ib, step, rk).x;
+    const uint32_t la = droplet_block_any(ia, step, rk).x, lb = droplet_block_any(ib, step, rk).x;
     return la < lb || (la == lb && ia < ib);
 }
 
@@ -159,7 +159,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
             if (m_src > kBoxChunkMax) __trap();           // the host admits n <= G * kBoxChunkMax, and n never grows
             for (int e = tid; e < m_src; e += kBoxThreads) {
                 const uint32_t i = (uint32_t)(lo + e);
-                const uint4 w = droplet_block(i, step, rk);
+                const uint4 w = droplet_block_any(i, step, rk);
                 const uint32_t d = __umulhi(w.y, G);
                 const int r = atomicAdd(&sm.cnt2[d], 1);
                 sm.rec0[e] = ((unsigned long long)w.y << 32) | i;
@@ -339,7 +339,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
             auto next_pair = [&](int &e, int &a, int &b, uint4 &w) -> bool {
                 for (; e < m && my_off + e + 1 < n; e += 2 * kBoxThreads) {
                     a = big ? ((volatile int *)idx)[my_off + e] : (int)(uint32_t)sm.rec0[e];
-                    w = droplet_block((uint32_t)a, step, rk);
+                    w = droplet_block_any((uint32_t)a, step, rk);
                     if (w.w > thr) continue;
                     if (e + 1 < m) {
                         b = big ? ((volatile int *)idx)[my_off + e + 1] : (int)(uint32_t)sm.rec0[e + 1];

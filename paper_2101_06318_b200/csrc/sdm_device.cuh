@@ -27,11 +27,14 @@ struct PhiloxKey {          // the ten round keys, precomputed once per thread (
     uint32_t k0[10], k1[10];
     uint32_t base;          // storage index of the handle's droplet 0 in the GLOBAL state (sdm_set_index_base): the
                             // Philox counter is base + local index, so a shard reproduces the unsharded stream
+    const unsigned long long *debug_keys;   // sdm_debug_permutation: sort keys supplied by the caller (by local storage
+                                            // index) instead of Philox words 0-1; NULL in every real step
 };
 
 __host__ __device__ __forceinline__ void philox_round_keys(uint64_t seed, uint32_t base, PhiloxKey &rk)
 {
     rk.base = base;
+    rk.debug_keys = nullptr;
     uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -61,6 +64,17 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 __device__ __forceinline__ uint4 droplet_block(uint32_t sid, uint64_t step, const PhiloxKey &rk)
 {
     return philox4x32_10(sid + rk.base, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
+}
+
+// The same, or -- in sdm_debug_permutation -- the caller's key in words 0-1 and a uniform of (almost) one.  Used by
+// every kernel except the fast section of k_fused_cells_count (which such a call does not enter).
+__device__ __forceinline__ uint4 droplet_block_any(uint32_t sid, uint64_t step, const PhiloxKey &rk)
+{
+    if (rk.debug_keys) {
+        const unsigned long long k = rk.debug_keys[sid];
+        return make_uint4((uint32_t)k, (uint32_t)(k >> 32), 0xFFFFFFFFu, 0xFFFFFFFFu);
+    }
+    return droplet_block(sid, step, rk);
 }
 
 __device__ __forceinline__ uint64_t block_key64(const uint4 &w)

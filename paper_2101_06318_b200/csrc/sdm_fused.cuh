@@ -116,10 +116,11 @@ __device__ __forceinline__ uint32_t flag_threshold(double P)
 // Works on shared memory only, so that the caller's register arrays never
 // get their address taken.  Called by the whole warp (every group with its own cell).
 __device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int N, int s, int n_s, int li, uint64_t seed,
-                                          uint32_t base, uint64_t step)
+                                          uint32_t base, uint64_t step, const unsigned long long *debug_keys = nullptr)
 {
     PhiloxKey rk;
     philox_round_keys(seed, base, rk);
+    rk.debug_keys = debug_keys;
     uint32_t mine[32], dst[32];
     for (int r = 0; r < E; ++r) {
         const int p = li * E + r;
@@ -132,12 +133,12 @@ __device__ __noinline__ void fix_key_ties(uint32_t *sk, int E, int N, int s, int
         while (b < n_s && ((sk[b] ^ me) < (uint32_t)N)) ++b;
         if (b - a < 2) continue;
         const int l = (int)(me & (uint32_t)(N - 1));
-        const uint64_t key = block_key64(droplet_block((uint32_t)(s + l), step, rk));
+        const uint64_t key = block_key64(droplet_block_any((uint32_t)(s + l), step, rk));
         int rank = 0;
         for (int q = a; q < b; ++q) {
             if (q == p) continue;
             const int l2 = (int)(sk[q] & (uint32_t)(N - 1));
-            const uint64_t key2 = block_key64(droplet_block((uint32_t)(s + l2), step, rk));
+            const uint64_t key2 = block_key64(droplet_block_any((uint32_t)(s + l2), step, rk));
             rank += key_less(key2, l2, key, l) ? 1 : 0;
         }
         dst[r] = (uint32_t)(a + rank);
@@ -182,7 +183,7 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
         const int a = (int)(sk[p] & (N - 1)), b = (int)(sk[p + 1] & (N - 1));
         // droplet a was element slot a / L of lane lane0 + a % L
         if (((sflag[a / L] >> (lane0 + a % L)) & 1u) == 0) continue;
-        const double u = block_uniform(droplet_block((uint32_t)(s + a), step, rk));
+        const double u = block_uniform(droplet_block_any((uint32_t)(s + a), step, rk));
         int64_t o0 = 0;
         double o1 = 0.0, o2 = 0.0;
         if (delta) pair_moments(xi, v, s + a, s + b, o0, o1, o2);
@@ -210,17 +211,19 @@ __device__ __noinline__ int collide_flagged(const uint32_t *sk, const uint32_t *
 template <bool TAB>
 __device__ __noinline__ int oversize_cell(int64_t *xi, double *v, int *idx, int s, int n_s, int lane,
                                           double dtdv, int32_t ktype, double kparam, uint64_t seed, uint32_t base,
-                                          uint64_t step, double *delta, const AttrView &av)
+                                          uint64_t step, double *delta, const AttrView &av,
+                                          const unsigned long long *debug_keys = nullptr)
 {
     PhiloxKey rk;
     philox_round_keys(seed, base, rk);
+    rk.debug_keys = debug_keys;
     warp_rank_by_counting(nullptr, s, n_s, s, idx, step, rk, lane);
     __syncwarp();
     const double norm = pair_norm(n_s, dtdv);
     int packed = 0;
     for (int q = lane; q < (n_s >> 1); q += 32) {
         int a = idx[s + 2 * q], b = idx[s + 2 * q + 1];
-        double u = block_uniform(droplet_block((uint32_t)a, step, rk));
+        double u = block_uniform(droplet_block_any((uint32_t)a, step, rk));
         int r = collide_pair_exact<TAB>(xi, v, a, b, u, norm, ktype, kparam, av);
         packed += (r & 1) + (((r >> 1) & 1) << 10) + (1 << 20);
     }
@@ -270,6 +273,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
     const int g = lane / L, li = lane % L, lane0 = g * L;
     PhiloxKey rk;
     philox_round_keys(prm.seed, prm.rk.base, rk);
+    rk.debug_keys = prm.rk.debug_keys;
     int events = 0, zeros = 0, exact = 0;
     const int cells_per_round = gridDim.x * kFusedWarps * G;
     for (int cbase = (blockIdx.x * kFusedWarps + warp) * G; cbase < n_cell; cbase += cells_per_round) {
@@ -284,7 +288,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
                 const int s2 = __shfl_sync(0xffffffffu, s, gg * L), n2 = __shfl_sync(0xffffffffu, n_s, gg * L);
                 if (n2 <= N) continue;
                 const int pk = oversize_cell<TAB>(xi, v, idx, s2, n2, lane, prm.dtdv, prm.kernel, prm.kparam,
-                                             prm.seed, prm.rk.base, prm.step, my_delta, prm.attr);
+                                             prm.seed, prm.rk.base, prm.step, my_delta, prm.attr, prm.rk.debug_keys);
                 events += pk & 1023; zeros += (pk >> 10) & 1023; exact += pk >> 20;
                 if (MOM) {
                     a0 += __double_as_longlong(my_delta[0]);
@@ -335,7 +339,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
         const uint32_t sid0 = (uint32_t)(s + li);
 #pragma unroll
         for (int k = 0; k < E; ++k) {
-            const uint4 w = droplet_block(sid0 + (uint32_t)(L * k), prm.step, rk);
+            const uint4 w = droplet_block_any(sid0 + (uint32_t)(L * k), prm.step, rk);
             const bool valid = nrem > L * k;
             x[k] = valid ? ((w.y & ~(uint32_t)(N - 1)) | (uint32_t)(li + L * k)) : 0xFFFFFFFFu;
             umin = min(umin, valid ? w.w : 0xFFFFFFFFu);
@@ -357,7 +361,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
 #pragma unroll
                 for (int r = 0; r < E; ++r) sk[li * E + r] = x[r];
                 __syncwarp();
-                fix_key_ties(sk, E, N, s, n_s, li, prm.seed, prm.rk.base, prm.step);
+                fix_key_ties(sk, E, N, s, n_s, li, prm.seed, prm.rk.base, prm.step, prm.rk.debug_keys);
 #pragma unroll
                 for (int r = 0; r < E; ++r) x[r] = sk[li * E + r];
                 __syncwarp();
@@ -392,7 +396,7 @@ k_fused_cells(int64_t *__restrict__ xi, double *__restrict__ v, const int *__res
             // redo the blocks of this lane's droplets to learn which ones are flagged
 #pragma unroll 1
             for (int k = 0; k < E; ++k) {
-                const uint4 w = droplet_block(sid0 + (uint32_t)(L * k), prm.step, rk);
+                const uint4 w = droplet_block_any(sid0 + (uint32_t)(L * k), prm.step, rk);
                 const uint32_t word = __ballot_sync(0xffffffffu, (nrem > L * k) && (w.w <= thr));
                 if (lane == (k & 31)) s_flags[warp][k] = word;
             }

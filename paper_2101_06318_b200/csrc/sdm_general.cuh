@@ -56,7 +56,7 @@ __device__ __forceinline__ void count_sort_ids(const int (&id)[E], int m, int la
         old[k] = 0;
         if (L * k < m) {                                               // warp-uniform: rows beyond the segment cost nothing
             const bool valid = nrem > L * k;
-            const uint4 w = droplet_block((uint32_t)id[k], step, rk);
+            const uint4 w = droplet_block_any((uint32_t)id[k], step, rk);
             const uint32_t hi = __funnelshift_l(w.x, w.y, shift);      // top 32 bits of key64 << shift
             if (valid) {
                 x[k] = (hi & ~(uint32_t)(N - 1)) | (uint32_t)(lane + L * k);
@@ -166,7 +166,7 @@ k_gen_count(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, int
             if (c >= 0 && leader) atomicAdd(priv ? &s_cnt[c] : &cell_cnt[c], __popc(peers));
             int seg = -1;
             if (c >= 0) {
-                const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
+                const uint4 w = droplet_block_any((uint32_t)i, prm.step, prm.rk);
                 seg = segment_of(c, w.y, cell_bits, bucket_base);
             }
             const unsigned speers = __match_any_sync(0xffffffffu, seg);
@@ -307,7 +307,7 @@ k_gen_scatter(const int32_t *__restrict__ cell, const Ctrl *__restrict__ ctrl, i
         const int c = cell[i];
         int b = c;
         if (split) {
-            const uint4 w = droplet_block((uint32_t)i, prm.step, prm.rk);
+            const uint4 w = droplet_block_any((uint32_t)i, prm.step, prm.rk);
             b = segment_of(c, w.y, cell_bits, bucket_base);
         }
         order[seg_start[b] + rank[i]] = i;
@@ -352,7 +352,7 @@ __device__ __forceinline__ int segment_pairs(const int *sorted, int s, int m, in
     const uint32_t thr = screen_threshold(prm, sb, n_s);
     for (int e = ((s - cs) & 1) + 2 * lane; e + 1 < m; e += 64) {
         const int a = sorted[e], b = sorted[e + 1];
-        const uint4 w = droplet_block((uint32_t)a, prm.step, prm.rk);
+        const uint4 w = droplet_block_any((uint32_t)a, prm.step, prm.rk);
         if (w.w > thr) continue;                          // u >= P >= p: gamma = 0, nothing to read
         const double u = block_uniform(w);
         const int r = collide_pair_exact<true>(xi, v, a, b, u, norm, prm.kernel, prm.kparam, prm.attr);
@@ -427,7 +427,7 @@ k_segment_sort_pairs(const int *__restrict__ seg_start, int n_seg, int split, in
                 for (int e = lane; e < P; e += 32) {
                     if (e < m) {
                         const int d = sm->ids[e];
-                        sm->key()[e] = block_key64(droplet_block((uint32_t)d, prm.step, rk));
+                        sm->key()[e] = block_key64(droplet_block_any((uint32_t)d, prm.step, rk));
                         sm->sid[e] = d;
                     } else {
                         sm->key()[e] = ~0ull;
@@ -478,7 +478,7 @@ k_pairs_straddle(const int *__restrict__ seg_start, int n_seg, const int *__rest
         if (cell[b] != c) continue;
         const int cs = cell_start[c];
         if ((p - 1 - cs) & 1) continue;                    // a is a second-in-pair
-        const uint4 w = droplet_block((uint32_t)a, prm.step, prm.rk);
+        const uint4 w = droplet_block_any((uint32_t)a, prm.step, prm.rk);
         if (w.w > screen_threshold(prm, sb, cell_start[c + 1] - cs)) continue;
         const double u = block_uniform(w);
         const int r = collide_pair_exact<true>(xi, v, a, b, u, pair_norm(cell_start[c + 1] - cs, prm.dtdv), prm.kernel,

@@ -298,11 +298,11 @@ __device__ __noinline__ void warp_rank_by_counting(const int *__restrict__ ids_i
 {
     for (int e = lane; e < m; e += 32) {
         int id = ids_in ? ids_in[e] : contiguous_base + e;
-        uint64_t key = block_key64(droplet_block((uint32_t)id, step, rk));
+        uint64_t key = block_key64(droplet_block_any((uint32_t)id, step, rk));
         int rank = 0;
         for (int f = 0; f < m; ++f) {
             int id2 = ids_in ? ids_in[f] : contiguous_base + f;
-            uint64_t key2 = block_key64(droplet_block((uint32_t)id2, step, rk));
+            uint64_t key2 = block_key64(droplet_block_any((uint32_t)id2, step, rk));
             rank += key_less(key2, id2, key, id) ? 1 : 0;
         }
         idx[out_base + rank] = id;
