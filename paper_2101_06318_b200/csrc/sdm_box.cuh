@@ -142,15 +142,15 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
     const PhiloxKey &rk = prm.rk;
     unsigned int epoch = 0;
     int events = 0, exact = 0;
+    int n = ((volatile Ctrl *)ctrl)->n;             // changes only in the in-launch compaction, which re-reads it
     for (int t = 0; t < n_steps; ++t) {
         const uint64_t step = prm.step + (uint64_t)t;
         const int p = t & 1, pc = t % 3;
         unsigned long long *q = queue + (long long)p * queue_stride;
-        int n, m_src, lo;
+        int m_src, lo;
         bool exact_layout = false;    // false: region d of the queue starts at d * region_cap; true: at its exact offset
         // ---------------- A: Philox, region histogram, records to the queue ----------------
         while (true) {
-            n = ((volatile Ctrl *)ctrl)->n;
             const int ch = (n + (int)G - 1) / (int)G;
             lo = min(n, c * ch);
             m_src = min(n, lo + ch) - lo;
@@ -194,6 +194,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
                     if (tid == 0) box->overflow[pc] = 0u;
                 }
                 box_grid_sync(box, G, epoch);
+                n = ((volatile Ctrl *)ctrl)->n;
                 continue;
             }
             if (!exact_layout && ((volatile unsigned int *)box->overflow)[pc] != 0u) {
