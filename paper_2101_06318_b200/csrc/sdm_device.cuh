@@ -61,9 +61,13 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 
 // counter = {global storage index lo, hi, step lo, hi}; global index = base + local index < 2^32 (checked by
 // sdm_set_index_base), so the hi word is 0
+__device__ __forceinline__ uint4 droplet_block_global(uint32_t gsid, uint64_t step, const PhiloxKey &rk)
+{
+    return philox4x32_10(gsid, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
+}
 __device__ __forceinline__ uint4 droplet_block(uint32_t sid, uint64_t step, const PhiloxKey &rk)
 {
-    return philox4x32_10(sid + rk.base, 0u, (uint32_t)step, (uint32_t)(step >> 32), rk);
+    return droplet_block_global(sid + rk.base, step, rk);
 }
 
 // The same, or -- in sdm_debug_permutation -- the caller's key in words 0-1 and a uniform of (almost) one.  Used by
