@@ -437,13 +437,26 @@ def main():
                                        "achieved": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9,
                                        "frac": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9 / peak}}
         else:
+            # general path (any storage order) and box path: the same 24 algorithmic bytes per droplet-step; what the
+            # gathers and scattered stores of shuffled storage cost on top counts against the implementation
+            whole = B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9
+            hbm_resident = 20 * w.n_sd > 2 * 126e6
             roofline = {"bound": "hbm", "kernel": ("k_box_steps (persistent box kernel; L2-resident workload)" if mode == 2
-                                                   else "k_segment_sort (general path; L2-resident workload)"),
-                        "achieved": None, "peak": peak, "unit": "GB/s", "frac": None, "traffic": None,
-                        "ms_per_launch": per_launch_s * 1e3, "launches_timed": kernel_n}
-    # traffic: DRAM bytes per launch of the dominant kernel from the committed ncu summary (C5 only)
-    if roofline is not None and mode == 1 and w.n_sd == 67108864:
-        roofline["traffic"] = ncu_dram_bytes(os.path.join(ROOT, "profiles", "r01_ncu_fused_kernel_c5.csv"))
+                                                   else "k_segment_sort_pairs (general path: sort + pairs of one segment per warp)"),
+                        "achieved": whole if hbm_resident else None, "peak": peak, "unit": "GB/s",
+                        "frac": whole / peak if hbm_resident else None, "traffic": None,
+                        "what": ("whole step (all launches of the general path) at 24 algorithmic bytes per droplet"
+                                 if hbm_resident else "L2-resident workload: no HBM roofline applies"),
+                        "peak_source": peak_src, "alg_bytes_per_droplet": B_ALG_STEP,
+                        "ms_per_launch": per_launch_s * 1e3, "launches_timed": kernel_n,
+                        "kernel_share_of_step": kernel_ms / ms if ms > 0 else None}
+    # traffic: DRAM bytes (read + write) per launch of the dominant kernel, from the committed ncu capture of this
+    # command (not measured in this run: a profiler is never attached to a timed run)
+    if roofline is not None and w.n_sd == 67108864:
+        src = {"C5": "r02_ncu_fused_kernel_c5.csv", "C5s": "r02_ncu_general_path_c5s.csv"}.get(args.workload)
+        if src is not None:
+            roofline["traffic"] = ncu_dram_bytes(os.path.join(ROOT, "profiles", src))
+            roofline["traffic_source"] = "profiles/" + src + " (ncu --set full capture of the same command)"
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -495,9 +495,34 @@ def test_every_shape_of_the_fused_kernel(sdm_mod, max_count, lanes):
     counts = rng.integers(0, max_count + 1, 37)
     counts[5], counts[11], counts[20] = max_count, 1, 0
     w = _ragged_workload(counts, seed=max_count, shuffled=False, kparam=0.3 / max_count)
-    opts = [(sdm_mod.OPT_LANES_PER_CELL, lanes)] if lanes else []
+    # the register-network kernel (SDM_OPT_SORT_ENGINE = 1): the automatic choice for cells <= 256 is the counting sort
+    opts = [(sdm_mod.OPT_SORT_ENGINE, 1)] + ([(sdm_mod.OPT_LANES_PER_CELL, lanes)] if lanes else [])
     events, _ = _run_parity(sdm_mod, w, 5, options=opts, expect_mode=1)
     assert events > 50
+
+
+def test_small_cells_sorted_in_groups(sdm_mod):
+    """Cells of <= 128 droplets go through the counting-sort kernel in GROUPS of up to 8 consecutive cells holding at
+    most 256 droplets together (cell number in the top bits of the sort word, pairs counted from each cell's start):
+    groups that fill the 256 slots exactly, empty cells inside and around groups, runs of more than 8 tiny cells,
+    odd cell sizes (pairs that start at odd group offsets), cells that must stay alone, the state's last group."""
+    counts = [64, 64, 64, 64, 0, 0, 0, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 100, 28, 128, 128, 0, 256, 3, 250, 6,
+              0, 0, 0, 0, 0, 0, 0, 0, 0, 5, 129, 127, 33, 31, 65, 63, 1, 0, 2, 17, 17, 17, 17, 17, 17, 17, 17, 17,
+              120, 120, 16, 200, 56, 0, 7, 9]
+    w = _ragged_workload(counts, seed=21, shuffled=False, kparam=0.004)
+    events, n_end = _run_parity(sdm_mod, w, 8, expect_mode=1)
+    assert events > 200 and n_end < w.n_sd
+
+
+def test_small_cells_in_a_large_table_take_tickets(sdm_mod):
+    """A table large enough for the chunk tickets (>= 32 cells per warp of the grid) made of small ragged cells: every
+    chunk is sorted in groups; two steps, whole state and permutation against the oracle."""
+    rng = np.random.default_rng(77)
+    counts = rng.integers(0, 41, 90000)
+    counts[::997] = 0
+    w = _ragged_workload(counts, seed=22, shuffled=False, kparam=0.02)
+    events, _ = _run_parity(sdm_mod, w, 2, expect_mode=1)
+    assert events > 1000
 
 
 @pytest.mark.parametrize("max_count,engine", [(256, 2), (256, 1), (200, 2), (100, 2), (31, 2)])
