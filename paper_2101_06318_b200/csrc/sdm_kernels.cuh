@@ -29,9 +29,10 @@ struct Ctrl {
     unsigned int moment_done;      // moments: last-block counter
     unsigned int compact_done;     // compaction: CTAs that have left the kernel
     unsigned int epoch;            // compaction: tag of valid tile status words (no clearing between calls)
-    int cell_ticket;               // per-cell kernel: dynamic work counter
-    int table_dirty;               // fused path: cell_start must be rebuilt from cell_id (set_state, or compaction moved droplets)
-    int pad0[1];
+    int cell_ticket[2];            // per-cell kernel: dynamic work counters; a launch draws from one and arms the other
+                                   // for the launch that follows (no re-arming launch in between)
+    int table_dirty;               // fused path: cell_start must be rebuilt from cell_id (compaction moved droplets and
+                                   // did not rebuild the table itself)
     unsigned long long n_events;   // pairs with gamma_tilde > 0
     unsigned long long n_exact;    // pairs whose Eq. 3 was evaluated in fp64
     // upper bounds over the WHOLE state for the probability screening of the general and box paths (sdm_general.cuh):
@@ -42,7 +43,7 @@ struct Ctrl {
     int scan_ticket;               // general path scan: tile ticket
     unsigned int scan_done;        // general path scan: CTAs that have left the kernel
     unsigned int scan_epoch;       // general path scan: tag of valid status words
-    int pad1;
+    unsigned int bar_gen;          // k_compact: generation of its grid barrier (compaction -> table rebuild)
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
@@ -319,16 +320,11 @@ __device__ __forceinline__ void cell_boundary(int prev, int c, int i, int *__res
     for (int cc = prev + 1; cc <= c; ++cc) cell_start[cc] = i;     // also fills empty cells
 }
 
-__global__ void __launch_bounds__(256)
-k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell,
-                    int *__restrict__ cell_start, int force, int ticket0)
+// Grid-wide: every thread of every CTA calls it (CTAs of 256 threads).
+__device__ __forceinline__ void cell_start_rebuild(const int32_t *__restrict__ cell, const Ctrl *ctrl, int n_cell,
+                                                   int *__restrict__ cell_start)
 {
-    // re-arm the chunk ticket of the step kernel that follows (its first gridDim*warps chunks are pre-assigned)
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->cell_ticket = ticket0;
-    // the previous step's kernel may already have derived this table from cell_id (sdm_fused_count.cuh,
-    // cell_table_from_staged_ids); it is stale only if a compaction has moved droplets since
-    if (!force && ctrl->table_dirty == 0) return;
-    const int n = ctrl->n;
+    const int n = ((volatile const Ctrl *)ctrl)->n;
     if (n == 0) {
         for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= n_cell; c += gridDim.x * blockDim.x)
             cell_start[c] = 0;
@@ -388,6 +384,22 @@ k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell,
     }
 }
 
+// Builds the table the fused path's first step after sdm_set_state / sdm_set_cell_id reads (later tables come out of
+// the step kernel itself, and out of k_compact when a compaction moves droplets); arms the chunk ticket of that step.
+__global__ void __launch_bounds__(256)
+k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell, int *__restrict__ cell_start, int ticket_sel,
+                    int ticket0)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->cell_ticket[ticket_sel] = ticket0; ctrl->table_dirty = 0; }
+    cell_start_rebuild(cell, ctrl, n_cell, cell_start);
+}
+
+// arms a chunk ticket when the step kernel's grid differs from the one the previous launch armed it for
+__global__ void k_arm_ticket(Ctrl *ctrl, int ticket_sel, int ticket0)
+{
+    ctrl->cell_ticket[ticket_sel] = ticket0;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Row a7: stable in-place stream compaction of xi == 0 (single pass, decoupled look-back)
 // ---------------------------------------------------------------------------------------------
@@ -410,10 +422,14 @@ struct CompactSmem {
     int s_tile, s_prefix;
 };
 
+// grid_wait (k_compact with a table to rebuild; needs every CTA of the launch resident): nobody returns before the last CTA
+// has published the new count -- a grid barrier, released through Ctrl::bar_gen.  table_rebuilt: the caller rebuilds the
+// fused path's cell table right after, so the table is not left marked dirty.
 template <class Sync>
 __device__ __forceinline__ void compact_tiles(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell,
                                               Ctrl *ctrl, unsigned long long *__restrict__ status, const AttrView &av,
-                                              CompactSmem &sm, double *s_extra, int tid, unsigned int n_ctas, Sync sync)
+                                              CompactSmem &sm, double *s_extra, int tid, unsigned int n_ctas, Sync sync,
+                                              bool grid_wait = false)
 {
     const int n = ((volatile Ctrl *)ctrl)->n;
     const unsigned long long tag = (unsigned long long)(((volatile Ctrl *)ctrl)->epoch & 0x3fffffffu) << 34;
@@ -503,27 +519,39 @@ __device__ __forceinline__ void compact_tiles(int64_t *__restrict__ xi, double *
     // zero_count and n before it counts itself out, so nobody sees the new values half-way
     sync();
     if (tid == 0) {
+        const unsigned int gen = ((volatile Ctrl *)ctrl)->bar_gen;      // read before this CTA counts itself out
         __threadfence();
         if (atomicAdd(&ctrl->compact_done, 1u) == n_ctas - 1) {
             __threadfence();
             ctrl->n = (n_tiles > 0) ? ((volatile Ctrl *)ctrl)->n_new : 0;
-            ctrl->table_dirty = 1;
+            ctrl->table_dirty = grid_wait ? 0 : 1;
             ctrl->zero_count = 0;
             ctrl->ticket = 0;
             ctrl->compact_done = 0;
             ctrl->epoch = ctrl->epoch + 1u;
+            __threadfence();
+            ((volatile Ctrl *)ctrl)->bar_gen = gen + 1u;
+        } else if (grid_wait) {
+            while (((volatile Ctrl *)ctrl)->bar_gen == gen) __nanosleep(64);
         }
+        __threadfence();
     }
+    if (grid_wait) sync();
 }
 
 __global__ void __launch_bounds__(kCompactThreads)
 k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict__ cell, Ctrl *ctrl,
-          unsigned long long *__restrict__ status, const AttrView av)
+          unsigned long long *__restrict__ status, const AttrView av, int *__restrict__ next_table, int n_cell)
 {
     extern __shared__ double s_extra[];                // av.n rows of kCompactTile values (extra attributes)
     __shared__ CompactSmem sm;
-    if (ctrl->zero_count == 0) return;                 // nothing to remove: every CTA leaves
-    compact_tiles(xi, v, cell, ctrl, status, av, sm, s_extra, (int)threadIdx.x, gridDim.x, [] { __syncthreads(); });
+    // nothing to remove: every CTA leaves (zero_count is cleared only after every CTA of a launch has read it)
+    if (((volatile Ctrl *)ctrl)->zero_count == 0) return;
+    // next_table (fused path, the host launches no more than the resident number of CTAs): the table the next step
+    // reads is rebuilt from the compacted cell ids in this launch, behind a grid barrier
+    compact_tiles(xi, v, cell, ctrl, status, av, sm, s_extra, (int)threadIdx.x, gridDim.x, [] { __syncthreads(); },
+                  next_table != nullptr);
+    if (next_table != nullptr) cell_start_rebuild(cell, ctrl, n_cell, next_table);
 }
 
 // ---------------------------------------------------------------------------------------------
