@@ -74,6 +74,12 @@ def build_workload(name: str, rank: int = 0, scale_cells: int | None = None):
         w = workloads.grid_uniform(nx, ny, 256, seed=rank)
         w.dV = 1.0                                 # collision-dense: p ~ 2.6e-2 per pair, the screening flags most cells
         return w, f"C5d: {nx}x{ny} cells x 256 droplets, gravitational kernel, dV = 1 (collision-dense), cell-contiguous"
+    if name == "C4x":                              # C4 at HBM scale: 1024x1024 cells of ~64 droplets (2^26), small cells in groups
+        return (workloads.grid_poisson(1024, 1024, 64.0, shuffled=False, seed=rank),
+                "C4x: 1024x1024 cells, Poisson(64)/cell (6.7e7 droplets), Golovin, cell-contiguous")
+    if name == "C5m":                              # C5 with 64 droplets per cell: 1024x1024 cells x 64
+        return (workloads.grid_uniform(1024, 1024, 64, seed=rank),
+                "C5m: 1024x1024 cells x 64 droplets, gravitational kernel, cell-contiguous")
     if name == "C4":
         return workloads.grid_poisson(shuffled=False, seed=rank), "C4: 128x128 cells, Poisson(64)/cell, Golovin, cell-contiguous"
     if name == "C4s":

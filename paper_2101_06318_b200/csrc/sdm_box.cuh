@@ -269,8 +269,8 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
             __threadfence();
             __syncthreads();
         } else if (m > 0) {
-            // sub-buckets of ~8 records: j = floor((key_hi - first key of the region) * S / width), monotone in the key
-            const int S = max(1, min(kBoxSubMax, (m + 7) >> 3));
+            // sub-buckets of ~3 records (at most 2048 of them): j = floor((key_hi - first key of the region) * S / width), monotone in the key
+            const int S = max(1, min(kBoxSubMax, (m + 2) / 3));
             const unsigned long long kb0 = (((unsigned long long)c << 32) + G - 1) / G;
             const unsigned long long kb1 = (((unsigned long long)(c + 1) << 32) + G - 1) / G;
             const unsigned long long M = ((unsigned long long)S << 32) / (kb1 - kb0);
