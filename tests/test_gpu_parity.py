@@ -255,6 +255,49 @@ def test_cell_scheduling_with_other_grid_sizes(sdm_mod, ctas_per_sm, edge, steps
     assert events > 500
 
 
+def test_steady_state_step_is_one_launch_and_grid_changes_rearm_the_ticket(sdm_mod):
+    """After the first step the fused path launches ONE kernel per sdm_coalescence_step (the previous launch left the
+    cell table and armed the chunk ticket) and one per sdm_remove_zero; changing the grid between steps
+    (SDM_OPT_CTAS_PER_SM) must re-arm the ticket (k_arm_ticket) and still give the oracle's result.  200 x 200 cells:
+    large enough for the ticket scheduler on one CTA per SM."""
+    w = workloads.grid_uniform(200, 200, 256, seed=12)
+    w.dV = 0.5
+    s = _make(sdm_mod, w, options=[(sdm_mod.OPT_CTAS_PER_SM, 1)])
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    launches = []
+    for step in range(5):
+        if step == 3:
+            s.set_option(sdm_mod.OPT_CTAS_PER_SM, 2)          # another grid: the armed ticket value no longer fits
+        before = s.counters()["launches"]
+        xi, v, cell, _ = _compare_step(s, xi, v, cell, w, step, fused_moments=(step % 2 == 0))
+        launches.append(s.counters()["launches"] - before)
+    # step 0: compaction + first table + step; steady state: compaction + step; step 3: + the re-arming launch
+    assert launches == [3, 2, 2, 3, 2], launches
+    s.close()
+
+
+def test_compaction_rebuilds_the_next_steps_table_in_its_own_launch(sdm_mod):
+    """C6-like cells (xi in {1,2,3}: droplets vanish every step) on the fused path: sdm_remove_zero moves droplets, so
+    the table the previous step's kernel left is stale and k_compact rebuilds it behind its grid barrier; no
+    k_cell_start_sorted launch after the first step.  cell_start, permutation and state against the oracle each step,
+    with cells that empty out completely and the state's last cells among them."""
+    rng = np.random.default_rng(5)
+    counts = rng.integers(1, 9, 3000)
+    counts[-40:] = 1                                           # the last cells empty out early
+    w = _ragged_workload(counts, seed=31, shuffled=False, kparam=0.2)
+    w.xi[:] = rng.integers(1, 3, w.n_sd)
+    s = _make(sdm_mod, w)
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    n0, launches = w.n_sd, []
+    for step in range(12):
+        before = s.counters()["launches"]
+        xi, v, cell, _ = _compare_step(s, xi, v, cell, w, step)
+        launches.append(s.counters()["launches"] - before)
+    assert len(xi) < 0.8 * n0                                  # real removals happened
+    assert launches[0] == 3 and all(k == 2 for k in launches[1:]), launches
+    s.close()
+
+
 # ---- ragged, degenerate and maximum-size segments --------------------------------------------------
 
 def _ragged_workload(counts, seed=0, shuffled=False, kparam=0.002):
