@@ -56,8 +56,10 @@ enum {
     SDM_OPT_SCREENING = 4,     /* [1] 0: evaluate Eq. 3 in fp64 for every pair (no fp32 pre-test)   */
     SDM_OPT_TIMING = 5,        /* [0] 1: bracket the dominant kernel of each step with CUDA events   */
     SDM_OPT_LANES_PER_CELL = 6, /* [0] 16: 16 lanes x 16 droplets for cells of 129..256 (tuning)         */
-    SDM_OPT_SORT_ENGINE = 7,   /* [0] fused path, per-cell permutation: 0 automatic, 1 register sorting  */
-                               /*     network, 2 bucket sort on the top key bits (cells <= 256 only)     */
+    SDM_OPT_SORT_ENGINE = 7,   /* [0] fused path, per-cell permutation: 0 automatic (counting sort on the */
+                               /*     top key bits when no cell exceeds 256 droplets -- small cells in    */
+                               /*     groups of up to 8 -- else the register sorting network), 1 the      */
+                               /*     network, 2 the counting sort (cells <= 256 only)                    */
     SDM_OPT_DETERMINISTIC = 8, /* [0] 1: cells are mapped to warps by a fixed rule (no work tickets), so the  */
                                /*     fp64 moment sums M1, M2 of sdm_coalescence_step_moments are reproducible */
                                /*     bit for bit from run to run (xi, v, idx, M0 always are)                 */
