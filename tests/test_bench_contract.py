@@ -42,3 +42,17 @@ def test_gpu_arm_fails_loudly_without_a_device():
         pytest.skip("a GPU is present")
     res = _run(["--steps", "1", "--warmup", "1", "--no-e2e", "--no-cpu-baseline"])
     assert res.returncode != 0 and "no CPU fallback" in (res.stderr + res.stdout)
+
+
+def test_roofline_traffic_comes_from_the_committed_ncu_summaries():
+    """bench.py reports roofline.traffic from the committed ncu captures (a profiler is never attached to a timed run)
+    and names the file: both summaries exist, parse, and are consistent with the algorithmic 24 B per droplet."""
+    sys.path.insert(0, ROOT)
+    import bench
+    n = 67108864
+    fused = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "r02_ncu_fused_kernel_c5.csv"))
+    general = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "r02_ncu_general_path_c5s.csv"))
+    assert fused is not None and general is not None
+    assert 0.9 < fused / (bench.B_ALG_FUSED_KERNEL * n) < 1.05         # the step kernel moves the algorithmic bytes, once
+    assert 1.5 < general / (bench.B_ALG_STEP * n) < 3.0                # shuffled storage: gathers and scattered stores on top
+    assert bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "missing.csv")) is None
