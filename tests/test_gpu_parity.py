@@ -351,6 +351,38 @@ def test_screening_off_gives_identical_results(sdm_mod):
     a.close(), b.close()
 
 
+def test_screening_bound_at_its_worst_case_pairs(sdm_mod):
+    """Below 40 um the gravitational kernel is 1.19e8 pi (r_j + r_k)^3 |r_j - r_k|, largest at r_k = r_j / 2, and the
+    screening bound of a cell uses exactly that maximum (27/16 R^4): cells made of droplets of radius R and R/2 only put
+    half of their pairs AT the bound.  With and without screening the states, event counts and moments must be
+    identical -- a bound a few per cent too low would drop events here -- and the screened run evaluates fewer pairs."""
+    import math
+    rng = np.random.default_rng(8)
+    n_cell, per = 96, 256
+    r = np.where(rng.random(n_cell * per) < 0.5, 30e-6, 15e-6)
+    v = (4.0 * math.pi / 3.0) * r ** 3
+    xi = np.full(n_cell * per, 10 ** 6, dtype=np.int64)
+    cell = np.repeat(np.arange(n_cell, dtype=np.int32), per)
+    w = workloads.Workload("worst_case_pairs", xi, v, cell, n_cell, 1.0, 2.0, workloads.configs.KERNEL_GRAVITATIONAL,
+                           1.0, 0, seed=5)
+    a = _make(sdm_mod, w)
+    b = _make(sdm_mod, w, options=[(sdm_mod.OPT_SCREENING, 0)])
+    for step in range(12):
+        for s in (a, b):
+            s.remove_zero(sync=False)
+            s.coalescence_step(w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    for ta, tb in zip(a.get_state(), b.get_state()):
+        assert torch.equal(ta, tb)
+    ca, cb = a.counters(), b.counters()
+    assert ca["events"] == cb["events"] > 2000
+    assert ca["exact_evals"] < 0.5 * cb["exact_evals"]
+    # and the oracle agrees with the unscreened run on the first step's outcome
+    x0, v0, c0 = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    _, _, nev = oracle.step(x0, v0, c0, n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, 0)
+    assert nev > 100
+    a.close(), b.close()
+
+
 def test_empty_and_single_droplet_states(sdm_mod):
     s = sdm_mod.SDM(16, 3)
     e64, ef, e32 = (torch.empty(0, dtype=t, device="cuda") for t in (torch.int64, torch.float64, torch.int32))
