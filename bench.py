@@ -170,12 +170,16 @@ def cpu_info():
     return model, os.cpu_count()
 
 
-def oracle_sample_rate(target_s: float = 12.0, full: bool = False):
+def oracle_sample_rate(target_s: float = 12.0, full: bool = False, full_workload=None):
     """The oracle as it stands, one thread, on a bounded C5-shaped sample (64x64 cells x 256), or -- with
-    --cpu-baseline-full -- three steps of the full-size C5 state (about a minute of CPU work)."""
+    --cpu-baseline-full, and by default when the run times at least 100 steps -- three steps of the full-size C5 state
+    (about 40 s of CPU work; SURVEY.md 8(d) "Oracle timing")."""
     import oracle
     import workloads
-    w = workloads.grid_uniform(512, 512, 256, seed=0) if full else workloads.grid_uniform(64, 64, 256, seed=0)
+    if full:
+        w = full_workload if full_workload is not None else workloads.grid_uniform(512, 512, 256, seed=0)
+    else:
+        w = workloads.grid_uniform(64, 64, 256, seed=0)
     if full:
         target_s = 1e9
     xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
@@ -466,9 +470,12 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        rate, osteps, on, oel = oracle_sample_rate(full=args.cpu_baseline_full)
+        # three steps of the full-size state when asked for, or when the run is long enough to afford them (the default
+        # 200-step run); the 2^20-droplet sample otherwise (short driver runs)
+        full = args.cpu_baseline_full or (args.workload == "C5" and args.cells is None and args.steps >= 100)
+        rate, osteps, on, oel = oracle_sample_rate(full=full, full_workload=w if args.workload == "C5" and args.cells is None else None)
         model, nproc = cpu_info()
-        shape = "full C5 state: 512x512" if args.cpu_baseline_full else "C5-shaped sample: 64x64"
+        shape = "full C5 state: 512x512" if full else "C5-shaped sample: 64x64"
         cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "cpu_model": model, "nproc": nproc,
                "sample": f"{shape} cells x 256 droplets (n_sd={on}), {osteps} steps in {oel:.1f} s, single thread"}
 
