@@ -56,3 +56,33 @@ def test_roofline_traffic_comes_from_the_committed_ncu_summaries():
     assert 0.9 < fused / (bench.B_ALG_FUSED_KERNEL * n) < 1.05         # the step kernel moves the algorithmic bytes, once
     assert 1.5 < general / (bench.B_ALG_STEP * n) < 3.0                # shuffled storage: gathers and scattered stores on top
     assert bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "missing.csv")) is None
+
+
+@pytest.mark.gpu
+def test_gpu_arm_prints_the_contract_line():
+    """The GPU arm on a small C5-shaped grid (64 x 64 cells): ONE JSON line with the keys of the bench contract --
+    throughput, device-timed step, clocks sampled under load, end-to-end through host buffers, launch count, roofline
+    of the dominant kernel and the oracle baseline."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    res = _run(["--gpus", "1", "--steps", "6", "--warmup", "3", "--cells", "64", "--e2e-steps", "1"])
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["metric"] == "super-droplet-steps/s" and d["unit"] == "sd-steps/s" and d["n_gpus"] == 1
+    assert d["steps"] == 6 and d["warmup"] == 3 and d["higher_is_better"] is True and d["scaling"] == "weak"
+    assert d["dtype"] == "f64" and d["data"] == "synthetic" and d["vs_baseline"] is None
+    n = d["config"]["n_sd_per_gpu"]
+    assert n == 64 * 64 * 256 and "workload" in d["config"] and "model" not in d["config"]
+    assert abs(d["value"] - n * 6 / (d["ms_per_step"] * 6e-3)) <= 1e-6 * d["value"]
+    assert d["gpu_launches"] == 2 * 6                      # steady state: sdm_remove_zero + the step kernel
+    assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(d["clocks"])
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == 20 * n and e["d2h_bytes_per_step"] >= 20 * n and 0 < e["value"] < d["value"]
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and 0 < r["frac"] < 1
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and r["alg_bytes_per_droplet"] == 24.0
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 1e5 and "sample" in c and "nproc" in c
