@@ -219,6 +219,32 @@ int sdm_remove_zero(sdm_t *h, int64_t *n_sd_out);
 int sdm_moments(sdm_t *h, int per_cell, int64_t *m0_dev, double *m1_dev, double *m2_dev);
 int sdm_moments_host(sdm_t *h, int per_cell, int64_t *m0_host, double *m1_host, double *m2_host);
 
+/* The global moments of sdm_moments(per_cell = 0) for callers that CANNOT allocate device memory -- no handle, no
+ * workspace, nothing to create or destroy.  Meant for code that owns (xi, v) on the device but has no way to get
+ * scratch memory when it wants the numbers: a host model whose own pool took the whole device at start-up, a
+ * monitoring hook on a thread that must not stall the device (cudaMalloc and cudaFree synchronise it), a plug-in in a
+ * process whose device-memory budget is fixed.  The partial sums and the arrival counter of the grid-wide reduction
+ * live in a static device array inside libsdm itself: SDM_NOALLOC_SCRATCH_BYTES on EVERY GPU that loads the library,
+ * held until the process exits.  The call itself performs no cudaMalloc, cudaFree or any other allocating call.
+ *   xi_dev[n_sd], v_dev[n_sd]  DEVICE pointers, 16-byte aligned, read only (may be NULL when n_sd == 0)
+ *   n_sd                       0 <= n_sd <= SDM_NOALLOC_MAX_SD (the kernels' 32-bit storage indices; the scratch need
+ *                              does not grow with n_sd); beyond it: SDM_ECAPACITY and a message naming the limit
+ *   m0_dev, m1_dev, m2_dev     DEVICE pointers to one int64 / double / double: M0 exact, M1 and M2 fp64 sums with the
+ *                              products rounded as (xi*v) and (xi*v)*v, equal to sdm_moments' to <= 1e-12 relative
+ *   cuda_stream                a cudaStream_t of the CURRENT device (NULL = legacy default stream); ASYNCHRONOUS
+ *   err_host, err_len          optional HOST buffer for a NUL-terminated message on failure (NULL / 0: none)
+ * The pointers and the stream must belong to the device that is current when the call is made.
+ * ONE ARRAY PER DEVICE IS SHARED BY ALL CALLS: calls that can overlap on the GPU (two streams, two threads) race on
+ * it and return wrong numbers; order them (one stream, or events).  The array keeps the previous call's contents;
+ * the call clears what has to start at zero and never reads a partial it did not write itself.
+ * The first call on a device looks up the array's device address (cudaGetSymbolAddress) and keeps it: make that first
+ * call before any stream capture begins.  Returns SDM_OK, SDM_EINVAL (negative n_sd, NULL or misaligned pointer),
+ * SDM_ECAPACITY (n_sd too large), SDM_ECUDA (no device, address look-up or launch failed). */
+#define SDM_NOALLOC_MAX_SD 2139095040 /* = SDM_MAX_CAPACITY */
+#define SDM_NOALLOC_SCRATCH_BYTES 28672 /* 256 B counter + 1184 CTAs x 3 partials x 8 B */
+int sdm_moments_noalloc(const int64_t *xi_dev, const double *v_dev, int64_t n_sd, int64_t *m0_dev, double *m1_dev,
+                        double *m2_dev, void *cuda_stream, char *err_host, size_t err_len);
+
 /* The spectrum product of Fig. 6: mass of droplets per unit of ln r [kg per m^3 of air per
  * unit ln r] on n_bins bins (1 <= n_bins <= SDM_MAX_BINS), all cells together.  Bin b holds the droplets with
  * v_edges_host[b] <= v < v_edges_host[b+1] (volumes, strictly increasing, n_bins + 1 values); its value is

@@ -28,4 +28,6 @@ from .binding import (  # noqa: F401
     library_path,
     workspace_bytes,
     version,
+    moments_noalloc,
+    NOALLOC_MAX_SD,
 )

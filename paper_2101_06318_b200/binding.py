@@ -39,6 +39,7 @@ SYMBOLS = (
     "sdm_get_permutation", "sdm_run", "sdm_get_counters", "sdm_get_timing", "sdm_last_error",
     "sdm_workspace_bytes_attr", "sdm_create_attr", "sdm_set_attributes", "sdm_get_attributes",
     "sdm_set_efficiency_table", "sdm_spectrum", "sdm_set_cell_id", "sdm_set_index_base", "sdm_set_kernel_source", "sdm_debug_permutation",
+    "sdm_moments_noalloc",
 )
 MAX_ATTR = 8
 
@@ -102,6 +103,7 @@ def load_library() -> C.CDLL:
     L.sdm_run.argtypes = [vp, dbl, dbl, C.POINTER(KernelDesc), u64, u64, i64, C.c_int]
     L.sdm_get_counters.argtypes = [vp, C.POINTER(i64)]
     L.sdm_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+    L.sdm_moments_noalloc.argtypes = [vp, vp, i64, vp, vp, vp, vp, C.c_char_p, C.c_size_t]
     L.sdm_last_error.argtypes = [vp]
     L.sdm_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -117,6 +119,36 @@ def version() -> int:
 
 def workspace_bytes(capacity: int, n_cell: int, n_attr: int = 1) -> int:
     return int(load_library().sdm_workspace_bytes_attr(capacity, n_cell, n_attr))
+
+
+NOALLOC_MAX_SD = 2139095040
+
+
+def moments_noalloc(xi, v, out, stream=None, n_sd=None):
+    """sdm_moments_noalloc: global moments of (xi, v) without a handle or a workspace, for code that cannot allocate
+    device memory when it needs them (everything on the device already belongs to someone's pool, or the thread must
+    not stall the device in cudaMalloc).  The reduction's scratch is a static 28 KiB array inside libsdm, one per GPU,
+    shared by every call: calls that may overlap on the GPU race, so keep them ordered (one stream).  Nothing is
+    allocated here either: `out` = (m0 int64[1], m1 float64[1], m2 float64[1]) device tensors supplied by the caller,
+    written asynchronously on `stream` (default: torch's current stream of xi's device).  n_sd defaults to len(xi).
+    The first call on a device should come before any stream capture."""
+    import torch
+
+    lib = load_library()
+    n = int(xi.shape[0] if n_sd is None else n_sd)
+    assert xi.is_cuda and v.is_cuda and xi.dtype == torch.int64 and v.dtype == torch.float64
+    assert xi.is_contiguous() and v.is_contiguous()
+    m0, m1, m2 = out
+    assert m0.is_cuda and m0.dtype == torch.int64 and m1.dtype == torch.float64 and m2.dtype == torch.float64
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(xi.device):
+        s = stream if stream is not None else torch.cuda.current_stream(xi.device)
+        rc = lib.sdm_moments_noalloc(C.c_void_p(xi.data_ptr()), C.c_void_p(v.data_ptr()), n, C.c_void_p(m0.data_ptr()),
+                                     C.c_void_p(m1.data_ptr()), C.c_void_p(m2.data_ptr()), C.c_void_p(s.cuda_stream),
+                                     err, len(err))
+    if rc != SDM_OK:
+        raise SdmError(rc, err.value.decode())
+    return out
 
 
 def _kernel(kernel: int, kparam: float) -> KernelDesc:
