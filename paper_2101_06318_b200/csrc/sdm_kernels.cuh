@@ -321,7 +321,17 @@ __device__ __forceinline__ void cell_boundary(int prev, int c, int i, int *__res
 }
 
 // Grid-wide: every thread of every CTA calls it (CTAs of 256 threads).
-__device__ __forceinline__ void cell_start_rebuild(const int32_t *__restrict__ cell, const Ctrl *ctrl, int n_cell,
+// kReadOnly = true: `cell` is not written by the launch that calls this (k_cell_start_sorted): streaming loads and the
+// non-coherent path (ld.global.nc) for the neighbour look-ups.  kReadOnly = false: the same launch rewrote `cell` in
+// place before a grid barrier (k_compact): ld.global.nc is only defined for data that stays read-only for the whole
+// kernel, and this SM may hold pre-barrier lines of the same addresses, so every read of `cell` goes to L2 (ld.cg).
+template <bool kReadOnly>
+__device__ __forceinline__ int4 cell_quad_load(const int4 *p) { return kReadOnly ? __ldcs(p) : __ldcg(p); }
+template <bool kReadOnly>
+__device__ __forceinline__ int cell_id_load(const int32_t *p) { return kReadOnly ? __ldg(p) : __ldcg(p); }
+
+template <bool kReadOnly>
+__device__ __forceinline__ void cell_start_rebuild(const int32_t *cell, const Ctrl *ctrl, int n_cell,
                                                    int *__restrict__ cell_start)
 {
     const int n = ((volatile const Ctrl *)ctrl)->n;
@@ -341,9 +351,9 @@ __device__ __forceinline__ void cell_start_rebuild(const int32_t *__restrict__ c
             int4 q[U];
             int pv[U];
 #pragma unroll
-            for (int u = 0; u < U; ++u) q[u] = __ldcs(cell4 + t0 + u * T);
+            for (int u = 0; u < U; ++u) q[u] = cell_quad_load<kReadOnly>(cell4 + t0 + u * T);
 #pragma unroll
-            for (int u = 0; u < U; ++u) pv[u] = (lane == 0) ? __ldg(cell + ((t0 + u * T) << 2) - 1) : 0;
+            for (int u = 0; u < U; ++u) pv[u] = (lane == 0) ? cell_id_load<kReadOnly>(cell + ((t0 + u * T) << 2) - 1) : 0;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int i = (t0 + u * T) << 2;
@@ -363,15 +373,15 @@ __device__ __forceinline__ void cell_start_rebuild(const int32_t *__restrict__ c
             if (t >= n4) break;
             int c0, c1, c2, c3;
             if (i + 3 < n) {
-                const int4 q = __ldcs(cell4 + t);
+                const int4 q = cell_quad_load<kReadOnly>(cell4 + t);
                 c0 = q.x; c1 = q.y; c2 = q.z; c3 = q.w;
             } else {                                                // the last, partial quad: repeat the last id
-                c0 = cell[i];
-                c1 = (i + 1 < n) ? cell[i + 1] : c0;
-                c2 = (i + 2 < n) ? cell[i + 2] : c1;
+                c0 = cell_id_load<kReadOnly>(cell + i);
+                c1 = (i + 1 < n) ? cell_id_load<kReadOnly>(cell + i + 1) : c0;
+                c2 = (i + 2 < n) ? cell_id_load<kReadOnly>(cell + i + 2) : c1;
                 c3 = c2;
             }
-            const int prev = (i > 0) ? __ldg(cell + i - 1) : -1;
+            const int prev = (i > 0) ? cell_id_load<kReadOnly>(cell + i - 1) : -1;
             if (prev != c3) {
                 if (c0 != prev) cell_boundary(prev, c0, i, cell_start);
                 if (c1 != c0) cell_boundary(c0, c1, i + 1, cell_start);
@@ -391,7 +401,7 @@ k_cell_start_sorted(const int32_t *__restrict__ cell, Ctrl *ctrl, int n_cell, in
                     int ticket0)
 {
     if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl->cell_ticket[ticket_sel] = ticket0; ctrl->table_dirty = 0; }
-    cell_start_rebuild(cell, ctrl, n_cell, cell_start);
+    cell_start_rebuild<true>(cell, ctrl, n_cell, cell_start);
 }
 
 // arms a chunk ticket when the step kernel's grid differs from the one the previous launch armed it for
@@ -551,7 +561,7 @@ k_compact(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restrict_
     // reads is rebuilt from the compacted cell ids in this launch, behind a grid barrier
     compact_tiles(xi, v, cell, ctrl, status, av, sm, s_extra, (int)threadIdx.x, gridDim.x, [] { __syncthreads(); },
                   next_table != nullptr);
-    if (next_table != nullptr) cell_start_rebuild(cell, ctrl, n_cell, next_table);
+    if (next_table != nullptr) cell_start_rebuild<false>(cell, ctrl, n_cell, next_table);   // `cell` was rewritten above
 }
 
 // ---------------------------------------------------------------------------------------------
