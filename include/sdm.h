@@ -69,6 +69,10 @@ enum {
                                /*     forces the overflow fallback to exact region offsets)                             */
     SDM_OPT_BOX_SORT_CAP = 12, /* [0] >0: largest region the box kernel sorts in shared memory (tests: a small value    */
                                /*     forces the ranking-by-counting fallback in global memory)                        */
+    SDM_OPT_COOPERATIVE = 13,  /* [1] 0: behave as on a device (or context) without cooperative launches: the compaction */
+                               /*     is a plain launch and the next step rebuilds its cell table, single-cell boxes take   */
+                               /*     the general path (tests; the library falls back to the same by itself when a         */
+                               /*     cooperative grid does not fit, e.g. under MPS)                                        */
     SDM_OPT_CTAS_PER_SM = 9    /* [0] >0: grid of the counting-sort kernel = value x SM count, at most 32      */
                                /*     (scaling runs; SDM_EINVAL if the grid would exceed the moment partials)  */
 };

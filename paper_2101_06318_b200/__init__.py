@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     OPT_BOX_CTAS,
     OPT_BOX_REGION_CAP,
     OPT_BOX_SORT_CAP,
+    OPT_COOPERATIVE,
     load_library,
     library_path,
     workspace_bytes,

@@ -26,6 +26,7 @@ OPT_CTAS_PER_SM = 9
 OPT_BOX_CTAS = 10
 OPT_BOX_REGION_CAP = 11
 OPT_BOX_SORT_CAP = 12
+OPT_COOPERATIVE = 13
 CNT_NAMES = ("n_sd", "events", "zeros", "launches", "mode", "max_cell", "exact_evals", "reserved")
 
 SDM_OK, SDM_EINVAL, SDM_ECAPACITY, SDM_ECUDA, SDM_ESTATE = 0, -1, -2, -3, -4

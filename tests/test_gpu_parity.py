@@ -298,6 +298,39 @@ def test_compaction_rebuilds_the_next_steps_table_in_its_own_launch(sdm_mod):
     s.close()
 
 
+def test_without_cooperative_launches_the_next_step_rebuilds_its_table(sdm_mod):
+    """SDM_OPT_COOPERATIVE = 0 stands for a device or context without cooperative launches (the library takes the same
+    branches by itself when a cooperative grid does not fit): k_compact is then a plain launch that cannot rebuild the
+    table the last step's kernel left, so the next fused step must not use that table -- it starts with
+    k_cell_start_sorted (3 launches per [remove_zero; step] instead of 2).  Same state as above: droplets vanish every
+    step and whole cells empty out.  A single-cell box takes the general path."""
+    rng = np.random.default_rng(5)
+    counts = rng.integers(1, 9, 3000)
+    counts[-40:] = 1
+    w = _ragged_workload(counts, seed=31, shuffled=False, kparam=0.2)
+    w.xi[:] = rng.integers(1, 3, w.n_sd)
+    s = _make(sdm_mod, w, options=[(sdm_mod.OPT_COOPERATIVE, 0)])
+    assert s.counters()["mode"] == 1
+    xi, v, cell = w.xi.copy(), w.v.copy(), w.cell_id.copy()
+    n0, launches = w.n_sd, []
+    for step in range(12):
+        before = s.counters()["launches"]
+        xi, v, cell, _ = _compare_step(s, xi, v, cell, w, step)
+        launches.append(s.counters()["launches"] - before)
+    assert len(xi) < 0.8 * n0
+    assert all(k == 3 for k in launches), launches
+    # sdm_run on the same handle: [remove_zero; step] x 6 without a host round trip in between
+    s.run(w.dt, w.dV, w.kernel, w.kparam, w.seed, 12, 6, True)
+    for step in range(12, 18):
+        xi, v, cell = oracle.remove_zero(xi, v, cell)
+        oracle.step(xi, v, cell, w.n_cell, w.dt, w.dV, w.kernel, w.kparam, w.seed, step)
+    gxi, gv, gc = (t.cpu().numpy() for t in s.get_state())
+    assert np.array_equal(gxi, xi) and np.array_equal(gv, v) and np.array_equal(gc, cell)
+    s.close()
+    wb = workloads.golovin_box(2 ** 12)
+    _run_parity(sdm_mod, wb, 6, options=[(sdm_mod.OPT_COOPERATIVE, 0)], expect_mode=0)
+
+
 # ---- ragged, degenerate and maximum-size segments --------------------------------------------------
 
 def _ragged_workload(counts, seed=0, shuffled=False, kparam=0.002):
