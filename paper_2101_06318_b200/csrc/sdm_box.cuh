@@ -70,7 +70,12 @@ constexpr size_t kBoxSmemBytes = sizeof(BoxSmem);
 
 // grid-wide barrier of a cooperative launch (all CTAs resident): monotone arrival counter, release/acquire through
 // __threadfence (which also drops stale L1 lines, as cooperative_groups' grid sync relies on)
-__device__ __forceinline__ void box_grid_sync(BoxCtrl *box, unsigned int G, unsigned int &epoch)
+// `after_acquire` runs in thread 0 only, between the acquire fence and the closing CTA barrier: the place to read a
+// global flag ONCE per CTA and publish it in shared memory, so that all threads of the CTA branch on the same value
+// (a flag that another CTA clears later must not be re-read by a slow warp: it would take a different path to the
+// next barrier).
+template <class F>
+__device__ __forceinline__ void box_grid_sync(BoxCtrl *box, unsigned int G, unsigned int &epoch, F after_acquire)
 {
     __syncthreads();
     epoch += 1;
@@ -80,8 +85,13 @@ __device__ __forceinline__ void box_grid_sync(BoxCtrl *box, unsigned int G, unsi
         const unsigned int target = epoch * G;
         while (*((volatile unsigned int *)&box->bar) < target) { }
         __threadfence();
+        after_acquire();
     }
     __syncthreads();
+}
+__device__ __forceinline__ void box_grid_sync(BoxCtrl *box, unsigned int G, unsigned int &epoch)
+{
+    box_grid_sync(box, G, epoch, [] {});
 }
 
 // exclusive scan of v[0..m) in shared memory by the whole CTA (m <= 2 * blockDim); out[m] = total
@@ -182,8 +192,15 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
                     if (pos < region_cap) q[(long long)d * region_cap + pos] = sm.rec0[e];
                 }
             }
-            box_grid_sync(box, G, epoch);                 // ---- every B of the previous step is complete; totals are final
-            if (remove_zero && ((volatile Ctrl *)ctrl)->zero_count != 0) {
+            // ---- every B of the previous step is complete; totals are final.  Thread 0 reads the two flags that decide
+            // the CTA's path once and publishes them: the last CTA to finish a compaction clears zero_count, and CTA 0
+            // clears the overflow flag, while a slow warp of another CTA may not have branched yet.
+            box_grid_sync(box, G, epoch, [&] {
+                sm.scalar[1] = remove_zero ? ((volatile Ctrl *)ctrl)->zero_count : 0;
+                sm.scalar[2] = (int)((volatile unsigned int *)box->overflow)[pc];
+            });
+            const int zeros_seen = sm.scalar[1], overflow_seen = sm.scalar[2];
+            if (zeros_seen != 0) {
                 // rare: step 0 of Fig. 3 inside the launch -- the stable compaction pass (warps 0-7), then phase A again
                 if (tid < kCompactThreads)
                     compact_tiles(xi, v, cell, ctrl, tile_status, prm.attr, csm, s_extra, tid, G,
@@ -197,7 +214,7 @@ k_box_steps(int64_t *__restrict__ xi, double *__restrict__ v, int32_t *__restric
                 n = ((volatile Ctrl *)ctrl)->n;
                 continue;
             }
-            if (!exact_layout && ((volatile unsigned int *)box->overflow)[pc] != 0u) {
+            if (!exact_layout && overflow_seen != 0) {
                 box_grid_sync(box, G, epoch);             // everybody has seen the flag
                 if (c == 0) {
                     for (int d = tid; d < (int)G; d += kBoxThreads) box->coltot[pc][d] = 0;
