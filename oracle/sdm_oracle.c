@@ -252,6 +252,11 @@ double orc_pair_probability(double K, int64_t xi_max, int64_t n_s, double dt, do
  * conversion to int64 (R8). */
 int64_t orc_gamma_tilde(double p, double u, int64_t xi_j, int64_t xi_k)
 {
+    /* DESIGN.md R20: Eq. 3 is a probability-like number >= 0 for every kernel of the paper.  A p that is not > 0
+     * (negative or NaN: only user-supplied kernel code can produce one) means "no event" -- without this the
+     * cast of NaN below would be undefined, and a negative gamma would make multiplicities grow.  For p = 0 the
+     * lines below give 0 as well, so nothing changes for p >= 0. */
+    if (!(p > 0.0)) return 0;
     double fl = floor(p);
     double gamma = fl + ((u < p - fl) ? 1.0 : 0.0);
     int64_t q = xi_j / xi_k;

@@ -101,3 +101,17 @@ def test_eq3_probability_against_exact_rational_formula():
     # the ratio is (n-1) for even n and n for odd n (R2)
     for n in range(2, 50):
         assert oracle.pair_probability(1.0, 1, n, 1.0, 1.0) == float(n - 1 if n % 2 == 0 else n)
+
+
+def test_gamma_tilde_of_a_probability_that_is_not_positive():
+    """DESIGN.md R20: p <= 0 or NaN (user kernel code returning a negative number or NaN) is 'no event', whatever the
+    uniform and the multiplicities; the smallest positive p still fires when phi allows it, and +inf is capped by
+    Eq. 4 (PAPER.md:104)."""
+    big = 10 ** 6
+    for p in (float("nan"), -float("nan"), -0.3, -1.0, -7.5, -1e300, -float("inf"), -0.0, 0.0):
+        for u in (0.0, 0.25, 0.999):
+            for xj, xk in ((big, 1), (9, 2), (3, 3)):
+                assert oracle.gamma_tilde(p, u, xj, xk) == 0, (p, u, xj, xk)
+    tiny = 5e-324
+    assert oracle.gamma_tilde(tiny, 0.0, big, 1) == 1 and oracle.gamma_tilde(tiny, 1e-300, big, 1) == 0
+    assert oracle.gamma_tilde(float("inf"), 0.5, 9, 2) == 4
