@@ -5,7 +5,7 @@
  * PAPER.md:<line>.  State of Fig. 2: per super-droplet a multiplicity xi
  * (int64), one extensive attribute, the volume v (fp64, m^3), and a cell id (int32).  Call order
  * and in/out intents follow Fig. 3.  Readings of the paper where it is silent
- * (RNG stream, tie rules, evaluation order, ...) are R1..R17 of DESIGN.md.
+ * (RNG stream, tie rules, evaluation order, ...) are R1..R20 of DESIGN.md.
  *
  * Conventions
  *  - Every entry point returns an int status: SDM_OK (0) or a negative SDM_E* code.  Nothing
@@ -171,7 +171,10 @@ int sdm_set_index_base(sdm_t *h, int64_t base);
  * every * and + of the user's code is rounded separately, like the library's own arithmetic) into one module with the
  * library's pair code (Eq. 3-6, Fig. 5); steps with SDM_KERNEL_USER build the permutation with the library's kernels and
  * evaluate every candidate pair through it (no probability screening: the library knows no bound of user code).
- * A user kernel that re-expresses a built-in one reproduces it bit for bit.  SYNCHRONOUS.  Errors: SDM_EINVAL (NULL
+ * A user kernel that re-expresses a built-in one reproduces it bit for bit.  The kernel should return a finite value
+ * >= 0; a pair whose Eq. 3 value p = a * xi_max * norm is not > 0 (the code returned a negative number or NaN) has no
+ * event, gamma_tilde = 0 (R20) -- multiplicities never grow.  +inf is capped by Eq. 4 like any large p.
+ * SYNCHRONOUS.  Errors: SDM_EINVAL (NULL
  * source, bad n_params, compilation failed: sdm_last_error holds the compiler log), SDM_ECUDA (NVRTC or the module loader
  * unavailable).  The kernel stays until replaced. */
 #define SDM_MAX_USER_PARAMS 16

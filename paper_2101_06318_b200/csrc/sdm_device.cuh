@@ -256,6 +256,9 @@ __device__ __forceinline__ int collide_pair_loaded(int64_t *__restrict__ xi, dou
                                    : coalescence_kernel(ktype, kparam, vj, vk);
 #endif
     double p = __dmul_rn(__dmul_rn(K, __ll2double_rn(xj)), norm);      // Eq. 3 in routine order (R3)
+#ifdef SDM_USER_KERNEL
+    if (!(p > 0.0)) return 0;                            // R20: user code returned a negative value or NaN: no event
+#endif
     double fl = floor(p);
     double gamma = (u < __dsub_rn(p, fl)) ? __dadd_rn(fl, 1.0) : fl;       // PAPER.md:102, R4
     if (gamma == 0.0) return 0;                          // gamma_tilde = min(0, q) = 0: the usual case, no division

@@ -88,6 +88,49 @@ def test_full_cells_counting_sort_kernel_and_an_asymmetric_kernel(sdm_mod):
     assert events > 200
 
 
+# R20: a kernel whose value is negative for some pairs, NaN for others (0/0) and a real collision rate for the rest
+BAD_VALUES = ("double sdm_user_kernel(double vj, double vk, const double *p) "
+              "{ double r = vj / vk; if (r > 1.5) return -p[0] * vj; if (r < 0.7) { double z = vj - vj; return z / z; } "
+              "return p[0] * (vj + vk); }")
+
+
+def test_negative_and_nan_kernel_values_are_no_event_on_every_path(sdm_mod):
+    """DESIGN.md R20.  Volumes spread over 0.5..2 so that all three branches of BAD_VALUES are taken by many pairs;
+    multiplicities never grow, events still happen, and device == oracle on the fused, general and box paths."""
+    rng = np.random.default_rng(8)
+    for shuffled, mode in ((False, 1), (True, 0)):
+        w = workloads.grid_small_multiplicity(16, 16, 32, seed=12, shuffled=shuffled)
+        w.v[:] = rng.uniform(0.5, 2.0, w.n_sd)
+        events, n_end = _run(sdm_mod, w, BAD_VALUES, [0.02], 8, expect_mode=mode)
+        assert events > 500 and n_end < w.n_sd
+    n = 5000
+    w = workloads.Workload("box", rng.integers(1, 4, n).astype(np.int64), rng.uniform(0.5, 2.0, n),
+                           np.zeros(n, dtype=np.int32), 1, 1.0, 1.0, 0, 0.0, 0, seed=4)
+    events, _ = _run(sdm_mod, w, BAD_VALUES, [2e-4], 6, expect_mode=2)
+    assert events > 300
+    # the three branches really occur among candidate pairs of such a state
+    r = w.v[0::2] / w.v[1::2]
+    assert (r > 1.5).sum() > 100 and (r < 0.7).sum() > 100 and ((r >= 0.7) & (r <= 1.5)).sum() > 100
+
+
+def test_permutation_pass_of_a_user_kernel_step_does_not_count_exact_evaluations(sdm_mod):
+    """With SDM_OPT_SCREENING = 0 the permutation pass in front of the user pair kernel (dt/dV = 0) used to evaluate and
+    count every pair a second time.  Now each candidate pair is counted once per step (give or take the 2^-31 chance
+    per droplet that its uniform word is 0 or 1)."""
+    w = workloads.grid_uniform(6, 6, 256, seed=3)
+    w.dV = 1.0
+    oracle.set_user_kernel(PRODUCT, [1e-30])
+    s = sdm_mod.SDM(w.n_sd, w.n_cell)
+    s.set_option(sdm_mod.OPT_SCREENING, 0)
+    s.set_kernel_source("__device__ " + PRODUCT, [1e-30])
+    s.set_state(_dev(w.xi), _dev(w.v), _dev(w.cell_id))
+    assert s.counters()["mode"] == 1
+    for step in range(3):
+        s.coalescence_step(w.dt, w.dV, sdm_mod.KERNEL_USER, 0.0, w.seed, step)
+    assert s.counters()["exact_evals"] == 3 * (w.n_sd // 2)
+    s.close()
+
+
 def test_golovin_as_user_code_reproduces_the_builtin_kernel_bit_for_bit(sdm_mod):
     w = workloads.grid_poisson(24, 24, 64.0, shuffled=False, seed=6)
     w.kparam = 1500.0 * 4000.0
