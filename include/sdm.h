@@ -271,7 +271,15 @@ int sdm_spectrum(sdm_t *h, int32_t n_bins, const double *v_edges_host, const dou
 int sdm_get_permutation(sdm_t *h, int32_t *idx_dev, int32_t *cell_start_dev);
 
 /* n_steps timesteps [sdm_remove_zero (if remove_zero_each_step); sdm_coalescence_step] with
- * step = step0, step0+1, ...; results equal the per-step calls.  ASYNCHRONOUS. */
+ * step = step0, step0+1, ...; results equal the per-step calls.  ASYNCHRONOUS.
+ *  - A single-cell box (n_cell == 1) with a built-in kernel runs all n_steps in ONE persistent launch.  With
+ *    SDM_KERNEL_USER (or when no cooperative grid fits the context) the call is a host loop of per-step launches.
+ *  - Shards (sdm_set_index_base): the index base is fixed for the whole call, while a removal in an EARLIER shard
+ *    shifts the global storage indices of this one.  With remove_zero_each_step != 0, a sharded run therefore equals
+ *    the unsharded run only as long as no earlier shard loses a droplet inside the call; from the first such removal
+ *    on it draws other random numbers (still a valid SDM realisation, no longer the same one).  For bit-for-bit
+ *    equality use the per-step calls and re-derive the bases after every removal (sharding.py: rebase), or verify
+ *    after the call that no shard's n_sd changed (bench.py does). */
 int sdm_run(sdm_t *h, double dt, double dV, const sdm_kernel_t *kernel, uint64_t seed,
             uint64_t step0, int64_t n_steps, int remove_zero_each_step);
 
