@@ -96,8 +96,9 @@ def build_workload(name: str, rank: int = 0, scale_cells: int | None = None):
 
 
 class ClockSampler:
-    """SM clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md): an NVML
-    polling thread (about one sample per millisecond, so even a 10 ms region is covered)."""
+    """SM clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md): an NVML polling thread that
+    reads the SM clock back to back (no sleep: a 6.5 ms region of 20 C5 steps still gets tens of samples) and the
+    throttle reasons and the board power on every fourth pass."""
 
     REASONS = (("hw_slowdown", "nvmlClocksEventReasonHwSlowdown"),
                ("hw_thermal_slowdown", "nvmlClocksEventReasonHwThermalSlowdown"),
@@ -133,15 +134,19 @@ class ClockSampler:
 
     def _poll(self):
         nv = self.nv
+        k = 0
         while not self.stop_flag.is_set():
             try:
                 self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
-                self.bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
-                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                if k % 4 == 0:
+                    self.bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception as e:                 # noqa: BLE001
                 self.error = str(e)
                 return
-            time.sleep(0.001)
+            k += 1
+            if len(self.sm) >= 200000:             # a seconds-long region: thin out instead of growing without bound
+                time.sleep(0.0005)
 
     def stop(self):
         if self.thread is None:
@@ -171,9 +176,8 @@ def cpu_info():
 
 
 def oracle_sample_rate(target_s: float = 12.0, full: bool = False, full_workload=None):
-    """The oracle as it stands, one thread, on a bounded C5-shaped sample (64x64 cells x 256), or -- with
-    --cpu-baseline-full, and by default when the run times at least 100 steps -- three steps of the full-size C5 state
-    (about 40 s of CPU work; SURVEY.md 8(d) "Oracle timing")."""
+    """The oracle as it stands, one thread: three steps of the full-size C5 state for the default workload (about 40 s
+    of CPU work; SURVEY.md 8(d) "Oracle timing"), a bounded C5-shaped sample (64x64 cells x 256) otherwise."""
     import oracle
     import workloads
     if full:
@@ -247,6 +251,9 @@ def main():
     ap.add_argument("--cpu-baseline-full", action="store_true",
                     help="time the oracle on 3 steps of the full-size C5 state instead of the 2^20 sample (~1 min)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the seconds-long steady-state region after the headline")
+    ap.add_argument("--sustained-seconds", type=float, default=3.0,
+                    help="full-size C5 on one GPU: length of the steady-state region timed after the headline region")
     ap.add_argument("--e2e-serial", action="store_true", help="e2e on ONE handle: H2D, step, D2H strictly one after the other")
     ap.add_argument("--e2e-shards", type=int, default=8, help="cell-range shards of the pipelined e2e measurement")
     ap.add_argument("--per-step-calls", action="store_true",
@@ -354,6 +361,35 @@ def main():
         ms = float(t.item())
     value = world * w.n_sd * args.steps / (ms * 1e-3)
 
+    # Steady state (MEASURED_PEAKS.json distinguishes burst from sustained): the headline region of the driver's
+    # --steps 20 is a 6.5 ms burst at ~260 W; over seconds the board reaches its power cap and the SM clock drops.  So
+    # the full-size C5 run goes on for >= --sustained-seconds more, timed the same way (CUDA events around the whole
+    # region, the library's own events around every launch of the dominant kernel), clocks sampled throughout.
+    sustained = None
+    if args.workload == "C5" and args.cells is None and world == 1 and mode == 1 and not args.no_sustained:
+        batch = 3000                               # sdm_get_timing keeps at most 4096 launches between two calls
+        n_batches = max(1, int(round(args.sustained_seconds * 1e3 / max(ms / args.steps, 1e-3) / batch)))
+        sus_sampler = ClockSampler(local)
+        sus_sampler.start()
+        sk_ms, sk_n, first = 0.0, 0, args.warmup + args.steps
+        sv0, sv1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        sv0.record()
+        for b in range(n_batches):
+            timed_steps(first + b * batch, batch)
+            k_ms, k_n = s.timing()                 # synchronises: one host round trip per 3000 steps (~1 s)
+            sk_ms, sk_n = sk_ms + k_ms, sk_n + k_n
+        sv1.record()
+        torch.cuda.synchronize()
+        sus_clocks = sus_sampler.stop()
+        sus_ms = sv0.elapsed_time(sv1)
+        sustained = {"steps": n_batches * batch, "seconds": sus_ms * 1e-3, "ms_per_step": sus_ms / (n_batches * batch),
+                     "kernel_ms": sk_ms / max(sk_n, 1), "launches_timed": sk_n,
+                     "sm_mhz_median": sus_clocks.get("sm_mhz"), "sm_mhz_min": sus_clocks.get("sm_mhz_min"),
+                     "power_w_median": sus_clocks.get("power_w"), "power_w_max": sus_clocks.get("power_w_max"),
+                     "clock_samples": sus_clocks.get("samples"), "reasons": sus_clocks.get("reasons")}
+        cnt = s.counters()
+
     # end to end through the C ABI with HOST buffers: H2D of the state, the step, D2H of the state
     e2e = None
     if not args.no_e2e:
@@ -446,6 +482,11 @@ def main():
                         "whole_step": {"alg_bytes_per_droplet": B_ALG_STEP,
                                        "achieved": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9,
                                        "frac": B_ALG_STEP * w.n_sd * args.steps / (ms * 1e-3) / 1e9 / peak}}
+            if sustained is not None:
+                # same algorithmic bytes, same peak: the fraction the kernel / the whole step keeps over seconds
+                sustained["frac"] = b_alg * w.n_sd / (sustained["kernel_ms"] * 1e-3) / 1e9 / peak
+                sustained["whole_step_frac"] = B_ALG_STEP * w.n_sd / (sustained["ms_per_step"] * 1e-3) / 1e9 / peak
+                roofline["sustained"] = sustained
         else:
             # general path (any storage order) and box path: the same 24 algorithmic bytes per droplet-step; what the
             # gathers and scattered stores of shuffled storage cost on top counts against the implementation
@@ -470,9 +511,9 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        # three steps of the full-size state when asked for, or when the run is long enough to afford them (the default
-        # 200-step run); the 2^20-droplet sample otherwise (short driver runs)
-        full = args.cpu_baseline_full or (args.workload == "C5" and args.cells is None and args.steps >= 100)
+        # three steps of the full-size C5 state whatever --steps is (SURVEY.md 8(d) "Oracle timing": C5, >= 3 steps;
+        # ~36 s of one host core); the 2^20-droplet sample for reduced grids and the other workloads
+        full = args.cpu_baseline_full or (args.workload == "C5" and args.cells is None)
         rate, osteps, on, oel = oracle_sample_rate(full=full, full_workload=w if args.workload == "C5" and args.cells is None else None)
         model, nproc = cpu_info()
         shape = "full C5 state: 512x512" if full else "C5-shaped sample: 64x64"
