@@ -44,6 +44,12 @@ def measured_peak_gbs():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+# committed ncu captures that roofline.traffic is read from, and the kernel sources each one describes (the contract test
+# fails when a source file has a later commit than its capture)
+TRAFFIC_SOURCES = {"C5": "r03_ncu_fused_kernel_c5.csv", "C5s": "r02_ncu_general_path_c5s.csv"}
+TRAFFIC_KERNEL_SOURCES = {"C5": ("sdm_fused_count.cuh", "sdm_fused.cuh"), "C5s": ("sdm_general.cuh",)}
+
+
 def ncu_dram_bytes(path):
     """dram__bytes_read.sum + dram__bytes_write.sum of the first captured launch in an ncu summary csv."""
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
@@ -504,7 +510,7 @@ def main():
     # traffic: DRAM bytes (read + write) per launch of the dominant kernel, from the committed ncu capture of this
     # command (not measured in this run: a profiler is never attached to a timed run)
     if roofline is not None and w.n_sd == 67108864:
-        src = {"C5": "r02_ncu_fused_kernel_c5.csv", "C5s": "r02_ncu_general_path_c5s.csv"}.get(args.workload)
+        src = TRAFFIC_SOURCES.get(args.workload)
         if src is not None:
             roofline["traffic"] = ncu_dram_bytes(os.path.join(ROOT, "profiles", src))
             roofline["traffic_source"] = "profiles/" + src + " (ncu --set full capture of the same command)"

@@ -50,12 +50,36 @@ def test_roofline_traffic_comes_from_the_committed_ncu_summaries():
     sys.path.insert(0, ROOT)
     import bench
     n = 67108864
-    fused = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "r02_ncu_fused_kernel_c5.csv"))
-    general = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "r02_ncu_general_path_c5s.csv"))
+    fused = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", bench.TRAFFIC_SOURCES["C5"]))
+    general = bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", bench.TRAFFIC_SOURCES["C5s"]))
     assert fused is not None and general is not None
     assert 0.9 < fused / (bench.B_ALG_FUSED_KERNEL * n) < 1.05         # the step kernel moves the algorithmic bytes, once
     assert 1.5 < general / (bench.B_ALG_STEP * n) < 3.0                # shuffled storage: gathers and scattered stores on top
     assert bench.ncu_dram_bytes(os.path.join(ROOT, "profiles", "missing.csv")) is None
+
+
+def test_roofline_traffic_captures_are_not_older_than_the_kernels_they_describe():
+    """roofline.traffic is read from a committed ncu capture, not measured in the run: it goes stale when the kernel
+    changes.  The commit that last touched a capture must not be older than the commit that last touched the kernel
+    source it describes (needs the git history: skipped in a snapshot without .git, e.g. on the GPU box)."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    def last_commit_time(rel):
+        res = subprocess.run(["git", "log", "-1", "--format=%ct", "--", rel], capture_output=True, text=True, cwd=ROOT)
+        out = res.stdout.strip()
+        return int(out) if res.returncode == 0 and out else None
+
+    if not os.path.isdir(os.path.join(ROOT, ".git")) or last_commit_time("bench.py") is None:
+        pytest.skip("no git history here")
+    for workload, capture in bench.TRAFFIC_SOURCES.items():
+        t_cap = last_commit_time(os.path.join("profiles", capture))
+        assert t_cap is not None, f"profiles/{capture} is not committed"
+        for src in bench.TRAFFIC_KERNEL_SOURCES[workload]:
+            t_src = last_commit_time(os.path.join("paper_2101_06318_b200", "csrc", src))
+            assert t_src is not None and t_cap >= t_src, (
+                f"profiles/{capture} (roofline.traffic of {workload}) is older than the last commit that touched {src}: "
+                "re-capture it (command in the .md beside it)")
 
 
 @pytest.mark.gpu
