@@ -43,3 +43,19 @@ def test_vj_is_the_volume_of_the_larger_multiplicity_hand_worked():
     xi, v = np.array([5, 2], dtype=np.int64), np.array([1.0, 1000.0])
     _, _, nev = oracle.step(xi, v, np.zeros(2, dtype=np.int32), 1, 1.0, 1.0, oracle.KERNEL_USER, 0.0, 0, 0)
     assert nev == 0 and xi.tolist() == [5, 2]
+
+
+def test_negative_and_nan_kernel_values_leave_the_pair_alone():
+    """DESIGN.md R20 through a whole step: user code that returns a negative number or NaN for some pairs produces no
+    event there -- the same two droplets as above, so the outcome is known by hand.  A negative value with the old
+    arithmetic gave gamma = -1 or 0 and xi_j = 5 + 2 = 7 (multiplicities growing); NaN reached an int64 cast."""
+    for body in ("return -1.0;", "double z = vj - vj; return z / z;", "return vj > vk ? -0.25 : 3.0;"):
+        oracle.set_user_kernel("double sdm_user_kernel(double vj, double vk, const double *p) { " + body + " }")
+        for seed in range(20):                      # whatever the uniform
+            xi, v = np.array([2, 5], dtype=np.int64), np.array([1.0, 1000.0])
+            _, _, nev = oracle.step(xi, v, np.zeros(2, dtype=np.int32), 1, 1.0, 1.0, oracle.KERNEL_USER, 0.0, seed, 0)
+            assert nev == 0 and xi.tolist() == [2, 5] and v.tolist() == [1.0, 1000.0], (body, seed)
+    # the third kernel is positive for the mirrored order (v_j = 1 < v_k = 1000): p = 3 * 5 = 15, cap floor(5/2) = 2
+    xi, v = np.array([5, 2], dtype=np.int64), np.array([1.0, 1000.0])
+    _, _, nev = oracle.step(xi, v, np.zeros(2, dtype=np.int32), 1, 1.0, 1.0, oracle.KERNEL_USER, 0.0, 0, 0)
+    assert nev == 1 and xi.tolist() == [1, 2] and v.tolist() == [1.0, 1002.0]
