@@ -132,11 +132,19 @@ class ClockSampler:
             nv.nvmlInit()
             self.nv, self.h = nv, self._handle(nv)
             self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM))
+            # the first call of each query can take milliseconds (lazy initialisation inside NVML): make it here, not in
+            # the polling thread, or a 6.5 ms timed region is over before the first sample arrives
+            nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+            nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+            nv.nvmlDeviceGetPowerUsage(self.h)
         except Exception as e:                     # noqa: BLE001
             self.error = f"NVML unavailable: {e}"
             return
         self.thread = threading.Thread(target=self._poll, daemon=True)
         self.thread.start()
+        t0 = time.perf_counter()                   # return once the thread is polling (bounded wait)
+        while not self.sm and self.error is None and time.perf_counter() - t0 < 0.5:
+            time.sleep(0.0002)
 
     def _poll(self):
         nv = self.nv
